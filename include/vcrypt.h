@@ -1,0 +1,152 @@
+/*
+ * vcrypt.h -- C ABI of libvcrypt: B200-native bit-level confusion + XOR video
+ * frame cipher ("Real-Time Bit-Level Encryption of Full High-Definition Video
+ * Without Diffusion", arxiv 2505.07158; PAPER.md).
+ *
+ * The calls follow the paper's problem statement: Algorithm 1's inputs
+ * (n, x0, y0, z0, w0, gamma, w, h) go to vcrypt_init, its loop
+ * body is vcrypt_encrypt_frames (plaintext frames in, ciphertext frames and
+ * the per-frame hash H out; the receiver is sent both), and the
+ * inverse transformation is vcrypt_decrypt_frames.
+ *
+ * Conventions
+ *   - Every function returns VCRYPT_OK (0) or a negative VCRYPT_E_* code; no
+ *     exception or abort crosses this boundary.  vcrypt_strerror names a code.
+ *   - The caller owns every buffer passed in or out.  "host" pointers may be
+ *     pageable or pinned (pinned buffers are copied from/to directly, pageable
+ *     ones are staged through the context's own pinned ring); "device"
+ *     pointers are plain CUDA device addresses on the context's device (for
+ *     instance torch.Tensor.data_ptr()), 16-byte aligned.
+ *   - Frames are H x W x 3 uint8, tightly packed (byte offset (i*W + j)*3 + c),
+ *     `n` frames back to back.  Hashes are n x 32 bytes in standard SHA-256
+ *     digest order.  Shift distances D are n x 3(H+W) uint16 with
+ *     D[c*(H+W) + i] = d_h(i,c) for i < H and D[c*(H+W) + H + j] = d_v(j,c);
+ *     keystream bytes B are n x H x W x 3 with the index of the pixel they mask.
+ *   - A context is stateful: the Lorenz hyper-chaotic main system LHCS_m is
+ *     chained from frame to frame, so each successful
+ *     vcrypt_encrypt_frames / vcrypt_decrypt_frames / vcrypt_derive call
+ *     advances the chain by the frames it processed; a failed call leaves the
+ *     chain where it was.  Encryption and decryption use separate contexts
+ *     created with the same parameters, and the decryptor must see the frames
+ *     in the same order from the first one.  One context per caller thread.
+ *   - Results never depend on `batch`, `n_streams`, `host_threads` or on which
+ *     kernel path (tiled / generic) a shape takes.
+ *   - There is no CPU fallback: without a CUDA device vcrypt_init fails with
+ *     VCRYPT_E_CUDA unless VCRYPT_FLAG_HOST_ONLY is set, in which case only the
+ *     host-side calls (vcrypt_frame_hash, vcrypt_derive, state accessors) work
+ *     and every call that needs the GPU returns VCRYPT_E_CUDA.
+ */
+#ifndef VCRYPT_H
+#define VCRYPT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define VCRYPT_OK 0
+#define VCRYPT_E_ARG (-1)    /* null pointer, zero size, misaligned device pointer   */
+#define VCRYPT_E_KEY (-2)    /* non-finite key word or gamma outside [-1.52, -0.06]  */
+#define VCRYPT_E_SHAPE (-3)  /* width/height/n_workers zero or too large             */
+#define VCRYPT_E_CUDA (-4)   /* CUDA error, or GPU call on a host-only context       */
+#define VCRYPT_E_NOMEM (-5)  /* host or device allocation failed                     */
+#define VCRYPT_E_STATE (-6)  /* chaotic state left the finite range                  */
+
+/* vcrypt_params.flags */
+#define VCRYPT_FLAG_HOST_ONLY 1u      /* no CUDA: host derivation hooks only (tests on CPU boxes)  */
+#define VCRYPT_FLAG_FORCE_GENERIC 2u  /* always take the any-shape gather kernels (test hook)     */
+#define VCRYPT_FLAG_HOST_SCALAR 4u    /* host derivation without SHA-NI / AVX lanes (test hook)   */
+
+typedef struct vcrypt_ctx vcrypt_ctx; /* opaque: chain state, host thread pool, streams, device and pinned buffers */
+
+typedef struct vcrypt_params {
+    double x0, y0, z0, w0;  /* the 256-bit key: initial values of LHCS_m (PAPER.md:85 Algo 1 inputs; Eq. 12 :449) */
+    double gamma;           /* control parameter, -1.52 <= gamma <= -0.06                           */
+    uint32_t n_workers;     /* protocol parameter n >= 1: sub-frame count and LHCS pair count;
+                               NOT the number of host threads                                                      */
+    uint32_t width, height; /* w, h; channels fixed at 3                                                          */
+    uint32_t batch;         /* frames per kernel launch in the host-buffer pipeline (0 -> 8)                      */
+    uint32_t n_streams;     /* pipeline depth: streams / staging slots (0 -> 3)                                   */
+    uint32_t host_threads;  /* host threads for hashing and derivation (0 -> hardware concurrency)                */
+    uint32_t flags;         /* VCRYPT_FLAG_*                                                                      */
+    int32_t device;         /* CUDA device ordinal (-1 -> current device)                                         */
+} vcrypt_params;
+
+/* Algorithm 1 set-up (PAPER.md:85 steps 1-2): validates the parameters, whitens the key (reading Q5 of
+ * N0 = 20000 RK4 steps), starts the host threads, creates streams and buffers.  The frame chain
+ * is at "first frame".  *out is written only on success. */
+int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p);
+
+/* Algorithm 1 steps 3-22 for n frames (hot-path rows a1-a11 of DESIGN.md):
+ * H = xor of the sub-frame SHA-256 hashes (:45), reconstruction of the initial values with H (:55), LHCS_m ->
+ * IR, worker systems -> D and B (:59), upload, bit-level confusion (Eq. 2, Eq. 3) and XOR (:75) on the GPU,
+ * download.  frames, cipher_out: host, n x H x W x 3 (cipher_out may equal frames).  hashes_out: host, n x 32. */
+int vcrypt_encrypt_frames(vcrypt_ctx *ctx, const uint8_t *frames, size_t n, uint8_t *cipher_out,
+                          uint8_t *hashes_out);
+
+/* The inverse transformation: the receiver holds the key and n and is sent F_e and H.
+ * cipher, plain_out: host, n x H x W x 3 (may alias).  hashes: host, n x 32, as returned by the encryptor. */
+int vcrypt_decrypt_frames(vcrypt_ctx *ctx, const uint8_t *cipher, const uint8_t *hashes, size_t n,
+                          uint8_t *plain_out);
+
+/* Waits for the context's GPU work, stops the host threads, frees everything.  NULL is allowed. */
+void vcrypt_destroy(vcrypt_ctx *ctx);
+
+/* Static string for a VCRYPT_* code. */
+const char *vcrypt_strerror(int code);
+
+/* Text of the last CUDA error a call on this context hit ("" if none); valid until the next failing call. */
+const char *vcrypt_last_cuda_error(const vcrypt_ctx *ctx);
+
+/* One-line description of the compiled-in constants of the method (integrator, dt, N0, K_m, u) and of the
+ * host code paths available on this CPU (SHA-NI, AVX-512 / AVX2 lanes).  Static string. */
+const char *vcrypt_describe(void);
+
+/* ---- host derivation hooks (work on host-only contexts) ------------------------------------------------ */
+
+/* H of one frame: sub-frame m = rows [floor(m*h/n), floor((m+1)*h/n)), H = xor_m SHA-256(f_m).
+ * frame: host, H x W x 3.  H_out: 32 bytes.  Does not touch the chain. */
+int vcrypt_frame_hash(vcrypt_ctx *ctx, const uint8_t *frame, uint8_t *H_out);
+
+/* Algorithm 1 steps 7-14 + Algorithm 2 steps 5-10 for one frame whose hash is `hash`:
+ * D_out (host, 3(H+W) uint16) and B_out (host, H x W x 3).  Advances the chain by one frame. */
+int vcrypt_derive(vcrypt_ctx *ctx, const uint8_t *hash, uint16_t *D_out, uint8_t *B_out);
+
+/* The chain state = last LHCS_m record (x_2n, y_2n, z_2n, w_2n) and the number of frames
+ * derived so far: 4 doubles + 1 counter are all a caller needs to checkpoint / resume a stream. */
+int vcrypt_get_state(const vcrypt_ctx *ctx, double state_out[4], uint64_t *frames_done);
+int vcrypt_set_state(vcrypt_ctx *ctx, const double state[4], uint64_t frames_done);
+
+/* Host threads actually started (the `cores` of a CPU-side figure). */
+int vcrypt_host_threads(const vcrypt_ctx *ctx);
+
+/* ---- kernel-only path: everything already resident in device memory ------------------------------------ */
+
+/* Algorithms 3-7 fused (rows a6-a10): for each of n frames
+ *   F_e(ro,j,c) = B(ro,j,c) xor hrot(F_o)(i0,j,c),  i0 = (ro - d_v(j,c) mod h) mod h,
+ * hrot = row i0 of channel c rotated by d_h(i0,c) mod 8w bit positions toward higher columns, LSB first.
+ * d_frames, d_B, d_cipher: device, n x H x W x 3; d_D: device, n x 3(H+W) uint16.  d_cipher may equal
+ * d_frames (in place); it must not partially overlap.  cuda_stream: a cudaStream_t (NULL = default stream).
+ * Asynchronous: returns after enqueueing; launch errors are reported, execution errors surface on sync. */
+int vcrypt_encrypt_device(vcrypt_ctx *ctx, const void *d_frames, const void *d_D, const void *d_B, size_t n,
+                          void *d_cipher, void *cuda_stream);
+
+/* Inverse of vcrypt_encrypt_device with the same D and B.  d_plain may equal d_cipher. */
+int vcrypt_decrypt_device(vcrypt_ctx *ctx, const void *d_cipher, const void *d_D, const void *d_B, size_t n,
+                          void *d_plain, void *cuda_stream);
+
+/* Number of kernels the last vcrypt_encrypt_device / vcrypt_decrypt_device call on this context launched,
+ * and since vcrypt_init in total (bench bookkeeping). */
+int vcrypt_launch_count(const vcrypt_ctx *ctx, uint64_t *last_call, uint64_t *total);
+
+/* Per-stage wall-clock of the last vcrypt_encrypt_frames / vcrypt_decrypt_frames call, milliseconds summed
+ * over its batches: [0] hashing, [1] chain + derivation, [2] staging copies on the host, [3] waiting for the GPU.
+ * (The paper's Fig. 13 phase split.) */
+int vcrypt_last_stage_ms(const vcrypt_ctx *ctx, double out[4]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VCRYPT_H */

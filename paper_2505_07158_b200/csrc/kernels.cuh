@@ -1,0 +1,53 @@
+// kernels.cuh -- launch interface of the sm_100a frame-cipher kernels (kernels.cu).
+// Internal to libvcrypt; the public boundary is include/vcrypt.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace vk {
+
+struct Geom {
+    uint32_t w, h;         // pixels
+    uint32_t row_bytes;    // 3w
+    uint32_t nD;           // 3(h+w) shift distances per frame
+    size_t frame_bytes;    // 3wh
+};
+
+inline Geom make_geom(uint32_t w, uint32_t h) {
+    Geom g;
+    g.w = w; g.h = h; g.row_bytes = 3u * w; g.nD = 3u * (h + w);
+    g.frame_bytes = (size_t)3u * w * h;
+    return g;
+}
+
+// Plan chosen once per context from (w, h) and the device's shared-memory size.
+struct Plan {
+    bool tiled;            // tiled two-pass path usable (w % 16 == 0 and a column strip fits in shared memory)
+    int strip_bytes;       // X: byte-columns per strip (128 / 64 / 32 / 16)
+    int strips_per_frame;  // ceil(3w / X)
+    int rows_per_block;    // row pass: rows a CTA stages at once
+    size_t smem_row;       // dynamic shared memory of the row pass
+    size_t smem_col;       // dynamic shared memory of the column pass
+    int col_ctas_per_sm;   // residency the column pass was sized for
+    size_t max_frames_per_launch;  // keeps the intermediate (n * 3wh bytes) L2-resident
+};
+
+cudaError_t make_plan(const Geom &g, int device, Plan *out);
+
+// Encrypt n frames: row pass (horizontal bit rotation, Eq. 2) then column pass
+// (vertical shift, Eq. 3, fused with the XOR of Algorithm 6).  dst may equal src.
+// Returns the number of kernels launched through *launches.
+cudaError_t encrypt_tiled(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
+                          size_t n, uint8_t *dst, cudaStream_t st, int *launches);
+cudaError_t decrypt_tiled(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
+                          size_t n, uint8_t *dst, cudaStream_t st, int *launches);
+
+// Any-shape path: one thread per output byte, closed-form gather straight from global memory.
+// dst must not alias src.
+cudaError_t encrypt_generic(const Geom &g, const uint8_t *src, const uint16_t *D, const uint8_t *B, size_t n,
+                            uint8_t *dst, cudaStream_t st, int *launches);
+cudaError_t decrypt_generic(const Geom &g, const uint8_t *src, const uint16_t *D, const uint8_t *B, size_t n,
+                            uint8_t *dst, cudaStream_t st, int *launches);
+
+}  // namespace vk

@@ -1,0 +1,501 @@
+// vcrypt.cpp -- the C ABI of include/vcrypt.h: context, host derivation driver, multi-stream pipeline.
+//
+// Algorithm 1 re-shaped for one B200: the main-thread loop over frames becomes a loop over
+// batches; the worker threads T_w of Algorithm 2 become jobs on a fixed thread pool (the protocol parameter n
+// fixes how the work is split, not how many threads run it); upload / GPU steps / download of a batch run on
+// one of `n_streams` CUDA streams while the host derives the next batch.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <chrono>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <memory>
+#include <new>
+#include <thread>
+#include <vector>
+
+#pragma GCC visibility push(default)
+#include "../../include/vcrypt.h"
+#pragma GCC visibility pop
+#include "host.hpp"
+#include "kernels.cuh"
+#include "thread_pool.hpp"
+
+namespace {
+
+using clk = std::chrono::steady_clock;
+inline double ms_since(clk::time_point t0) { return std::chrono::duration<double, std::milli>(clk::now() - t0).count(); }
+
+struct Slot {
+    cudaStream_t st = nullptr;
+    cudaEvent_t done = nullptr;
+    // pinned staging (h_F / h_out only when the caller's buffers are pageable)
+    uint8_t *h_F = nullptr, *h_B = nullptr, *h_out = nullptr;
+    uint16_t *h_D = nullptr;
+    // device
+    uint8_t *d_F = nullptr, *d_B = nullptr, *d_out = nullptr;  // d_out only on the any-shape kernel path
+    uint16_t *d_D = nullptr;
+    // work in flight
+    bool busy = false;
+    uint8_t *user_out = nullptr;  // where h_out goes once `done` fires (nullptr: D2H went straight to the caller)
+    size_t out_bytes = 0;
+};
+
+}  // namespace
+
+struct vcrypt_ctx {
+    vcrypt_params p{};
+    vk::Geom g{};
+    vk::Plan plan{};
+    bool cuda = false;
+    int device = -1;
+    bool simd = true;
+    int isa = 0;
+    double S[4] = {0, 0, 0, 0};
+    uint64_t frames_done = 0;
+    std::unique_ptr<vh::ThreadPool> pool;
+    size_t batch = 8;
+    std::vector<Slot> slots;
+    // per-batch host scratch
+    std::vector<double> IR;               // batch x 2n x 4
+    std::vector<vh::WorkerSlice> slices;  // batch x n
+    std::vector<uint8_t> subhash;         // batch x n x 32
+    // generic-path scratch for in-place calls
+    uint8_t *d_scratch = nullptr;
+    size_t scratch_bytes = 0;
+    // bookkeeping
+    uint64_t launches_last = 0, launches_total = 0;
+    double stage_ms[4] = {0, 0, 0, 0};
+    char cuda_msg[256] = {0};
+};
+
+namespace {
+
+int cuda_fail(vcrypt_ctx *c, cudaError_t e, const char *what) {
+    if (c) std::snprintf(c->cuda_msg, sizeof c->cuda_msg, "%s: %s", what, cudaGetErrorString(e));
+    return VCRYPT_E_CUDA;
+}
+#define VC_CUDA(ctx, call)                                           \
+    do {                                                             \
+        cudaError_t e__ = (call);                                    \
+        if (e__ != cudaSuccess) return cuda_fail((ctx), e__, #call); \
+    } while (0)
+
+bool is_pinned(const void *p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeHost;
+}
+
+void free_slot(Slot &s) {
+    if (s.st) cudaStreamSynchronize(s.st);
+    if (s.h_F) cudaFreeHost(s.h_F);
+    if (s.h_B) cudaFreeHost(s.h_B);
+    if (s.h_out) cudaFreeHost(s.h_out);
+    if (s.h_D) cudaFreeHost(s.h_D);
+    if (s.d_F) cudaFree(s.d_F);
+    if (s.d_B) cudaFree(s.d_B);
+    if (s.d_out) cudaFree(s.d_out);
+    if (s.d_D) cudaFree(s.d_D);
+    if (s.done) cudaEventDestroy(s.done);
+    if (s.st) cudaStreamDestroy(s.st);
+    s = Slot{};
+}
+
+// Device + pinned buffers of one slot, allocated on first use so that contexts used only through the
+// *_device calls or the host hooks stay cheap.
+int ensure_slot(vcrypt_ctx *c, Slot &s, bool need_hF, bool need_hout) {
+    const size_t fb = c->g.frame_bytes * c->batch, db = (size_t)c->g.nD * c->batch * sizeof(uint16_t);
+    if (!s.st) VC_CUDA(c, cudaStreamCreateWithFlags(&s.st, cudaStreamNonBlocking));
+    if (!s.done) VC_CUDA(c, cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+    if (!s.d_F) VC_CUDA(c, cudaMalloc(&s.d_F, fb));
+    if (!s.d_B) VC_CUDA(c, cudaMalloc(&s.d_B, fb));
+    const bool generic = !c->plan.tiled || (c->p.flags & VCRYPT_FLAG_FORCE_GENERIC);
+    if (generic && !s.d_out) VC_CUDA(c, cudaMalloc(&s.d_out, fb));
+    if (!s.d_D) VC_CUDA(c, cudaMalloc(&s.d_D, db));
+    if (!s.h_B) VC_CUDA(c, cudaHostAlloc(&s.h_B, fb, cudaHostAllocDefault));
+    if (!s.h_D) VC_CUDA(c, cudaHostAlloc(&s.h_D, db, cudaHostAllocDefault));
+    if (need_hF && !s.h_F) VC_CUDA(c, cudaHostAlloc(&s.h_F, fb, cudaHostAllocDefault));
+    if (need_hout && !s.h_out) VC_CUDA(c, cudaHostAlloc(&s.h_out, fb, cudaHostAllocDefault));
+    return VCRYPT_OK;
+}
+
+// Waits for a slot's GPU work and hands staged output to the caller.
+int retire_slot(vcrypt_ctx *c, Slot &s) {
+    if (!s.busy) return VCRYPT_OK;
+    const auto t0 = clk::now();
+    VC_CUDA(c, cudaEventSynchronize(s.done));
+    c->stage_ms[3] += ms_since(t0);
+    s.busy = false;
+    if (s.user_out) {
+        const auto t1 = clk::now();
+        const size_t chunk = (size_t)1 << 20, nch = (s.out_bytes + chunk - 1) / chunk;
+        uint8_t *dst = s.user_out;
+        const uint8_t *src = s.h_out;
+        const size_t total = s.out_bytes;
+        c->pool->parallel_for(nch, [&](size_t i) {
+            const size_t o = i * chunk, len = total - o < chunk ? total - o : chunk;
+            std::memcpy(dst + o, src + o, len);
+        });
+        c->stage_ms[2] += ms_since(t1);
+        s.user_out = nullptr;
+    }
+    return VCRYPT_OK;
+}
+
+int launch_cipher(vcrypt_ctx *c, bool decrypt, const uint8_t *src, const uint16_t *D, const uint8_t *B, size_t n,
+                  uint8_t *dst, cudaStream_t st) {
+    int launches = 0;
+    cudaError_t e;
+    const bool aligned = ((((uintptr_t)src) | ((uintptr_t)dst) | ((uintptr_t)B)) & 15u) == 0;
+    if (c->plan.tiled && aligned && !(c->p.flags & VCRYPT_FLAG_FORCE_GENERIC)) {
+        e = decrypt ? vk::decrypt_tiled(c->g, c->plan, src, D, B, n, dst, st, &launches)
+                    : vk::encrypt_tiled(c->g, c->plan, src, D, B, n, dst, st, &launches);
+    } else {
+        uint8_t *out = dst;
+        const size_t bytes = n * c->g.frame_bytes;
+        if (dst == src) {  // the gather kernels cannot run in place: go through scratch
+            if (c->scratch_bytes < bytes) {
+                if (c->d_scratch) {
+                    VC_CUDA(c, cudaStreamSynchronize(st));
+                    VC_CUDA(c, cudaFree(c->d_scratch));
+                    c->d_scratch = nullptr;
+                    c->scratch_bytes = 0;
+                }
+                VC_CUDA(c, cudaMalloc(&c->d_scratch, bytes));
+                c->scratch_bytes = bytes;
+            }
+            out = c->d_scratch;
+        }
+        e = decrypt ? vk::decrypt_generic(c->g, src, D, B, n, out, st, &launches)
+                    : vk::encrypt_generic(c->g, src, D, B, n, out, st, &launches);
+        if (e == cudaSuccess && out != dst) e = cudaMemcpyAsync(dst, out, bytes, cudaMemcpyDeviceToDevice, st);
+    }
+    c->launches_last += (uint64_t)launches;
+    c->launches_total += (uint64_t)launches;
+    if (e != cudaSuccess) return cuda_fail(c, e, decrypt ? "decrypt launch" : "encrypt launch");
+    return VCRYPT_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+// context life cycle
+// =====================================================================================================
+extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
+    if (!out || !p) return VCRYPT_E_ARG;
+    if (!std::isfinite(p->x0) || !std::isfinite(p->y0) || !std::isfinite(p->z0) || !std::isfinite(p->w0)) return VCRYPT_E_KEY;
+    const double lim = 9007199254740992.0;  // 2^53: integer parts stay exact
+    if (std::fabs(p->x0) >= lim || std::fabs(p->y0) >= lim || std::fabs(p->z0) >= lim || std::fabs(p->w0) >= lim) return VCRYPT_E_KEY;
+    if (!(p->gamma >= -1.52 && p->gamma <= -0.06)) return VCRYPT_E_KEY;
+    if (p->n_workers == 0 || p->width == 0 || p->height == 0) return VCRYPT_E_SHAPE;
+    if (p->n_workers > (1u << 20) || p->width > (1u << 16) || p->height > (1u << 16)) return VCRYPT_E_SHAPE;
+    vcrypt_ctx *c = new (std::nothrow) vcrypt_ctx;
+    if (!c) return VCRYPT_E_NOMEM;
+    int rc = VCRYPT_OK;
+    try {
+        c->p = *p;
+        c->g = vk::make_geom(p->width, p->height);
+        c->batch = p->batch ? p->batch : 8;
+        c->simd = !(p->flags & VCRYPT_FLAG_HOST_SCALAR);
+        c->isa = c->simd ? vh::best_isa() : 0;
+        unsigned nt = p->host_threads ? p->host_threads : std::thread::hardware_concurrency();
+        if (nt < 1) nt = 1;
+        if (nt > 256) nt = 256;
+        c->pool.reset(new vh::ThreadPool(nt));
+        // reading Q5: one-off key whitening
+        c->S[0] = p->x0; c->S[1] = p->y0; c->S[2] = p->z0; c->S[3] = p->w0;
+        for (int k = 0; k < vh::kWhiten; ++k) vh::rk4_step(c->S, p->gamma);
+        if (!vh::finite4(c->S)) rc = VCRYPT_E_STATE;
+        c->IR.resize(c->batch * 2u * p->n_workers * 4u);
+        c->slices.resize(c->batch * (size_t)p->n_workers);
+        c->subhash.resize(c->batch * (size_t)p->n_workers * 32u);
+        if (rc == VCRYPT_OK && !(p->flags & VCRYPT_FLAG_HOST_ONLY)) {
+            int dev = p->device;
+            cudaError_t e = cudaSuccess;
+            if (dev < 0) e = cudaGetDevice(&dev);
+            if (e == cudaSuccess) e = cudaSetDevice(dev);
+            if (e == cudaSuccess) e = vk::make_plan(c->g, dev, &c->plan);
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                rc = VCRYPT_E_CUDA;
+            } else {
+                c->cuda = true;
+                c->device = dev;
+                c->slots.resize(p->n_streams ? p->n_streams : 3);
+            }
+        }
+    } catch (const std::bad_alloc &) {
+        rc = VCRYPT_E_NOMEM;
+    } catch (...) {
+        rc = VCRYPT_E_ARG;
+    }
+    if (rc != VCRYPT_OK) {
+        delete c;
+        return rc;
+    }
+    *out = c;
+    return VCRYPT_OK;
+}
+
+extern "C" void vcrypt_destroy(vcrypt_ctx *c) {
+    if (!c) return;
+    if (c->cuda) {
+        cudaSetDevice(c->device);
+        for (Slot &s : c->slots) free_slot(s);
+        if (c->d_scratch) {
+            cudaDeviceSynchronize();
+            cudaFree(c->d_scratch);
+        }
+    }
+    delete c;
+}
+
+extern "C" const char *vcrypt_strerror(int code) {
+    switch (code) {
+        case VCRYPT_OK: return "ok";
+        case VCRYPT_E_ARG: return "invalid argument (null pointer, zero size or misaligned device pointer)";
+        case VCRYPT_E_KEY: return "invalid key (non-finite word, or gamma outside [-1.52, -0.06])";
+        case VCRYPT_E_SHAPE: return "invalid shape (width, height or n_workers zero or too large)";
+        case VCRYPT_E_CUDA: return "CUDA error, or GPU call on a host-only context";
+        case VCRYPT_E_NOMEM: return "out of memory";
+        case VCRYPT_E_STATE: return "chaotic state left the finite range";
+        default: return "unknown vcrypt error code";
+    }
+}
+
+extern "C" const char *vcrypt_describe(void) {
+    static char buf[384];
+    static bool done = false;
+    if (!done) {
+        std::snprintf(buf, sizeof buf,
+                      "vcrypt: LHCS sigma=10 rho=28 beta=8/3, RK4 dt=%.3f, whitening N0=%d steps, IR record stride K_m=%d, "
+                      "bound u=%llu, 6 mantissa bytes per variable; host: sha_ni=%d lanes_isa=%d (0 scalar, 1 avx2x4, 2 avx512x8); "
+                      "device: sm_100a tiled row pass + column pass, any-shape gather",
+                      vh::kDt, vh::kWhiten, vh::kRecordStride, (unsigned long long)vh::kBound, (int)vh::cpu_has_shani(),
+                      vh::best_isa());
+        done = true;
+    }
+    return buf;
+}
+
+extern "C" const char *vcrypt_last_cuda_error(const vcrypt_ctx *c) { return c ? c->cuda_msg : ""; }
+
+extern "C" int vcrypt_get_state(const vcrypt_ctx *c, double state_out[4], uint64_t *frames_done) {
+    if (!c || !state_out) return VCRYPT_E_ARG;
+    std::memcpy(state_out, c->S, sizeof c->S);
+    if (frames_done) *frames_done = c->frames_done;
+    return VCRYPT_OK;
+}
+
+extern "C" int vcrypt_set_state(vcrypt_ctx *c, const double state[4], uint64_t frames_done) {
+    if (!c || !state) return VCRYPT_E_ARG;
+    if (!vh::finite4(state)) return VCRYPT_E_STATE;
+    std::memcpy(c->S, state, sizeof c->S);
+    c->frames_done = frames_done;
+    return VCRYPT_OK;
+}
+
+extern "C" int vcrypt_host_threads(const vcrypt_ctx *c) { return c ? (int)c->pool->size() : VCRYPT_E_ARG; }
+
+extern "C" int vcrypt_launch_count(const vcrypt_ctx *c, uint64_t *last_call, uint64_t *total) {
+    if (!c) return VCRYPT_E_ARG;
+    if (last_call) *last_call = c->launches_last;
+    if (total) *total = c->launches_total;
+    return VCRYPT_OK;
+}
+
+extern "C" int vcrypt_last_stage_ms(const vcrypt_ctx *c, double out[4]) {
+    if (!c || !out) return VCRYPT_E_ARG;
+    std::memcpy(out, c->stage_ms, sizeof c->stage_ms);
+    return VCRYPT_OK;
+}
+
+// =====================================================================================================
+// host derivation (Algorithm 1 steps 4-14, Algorithm 2)
+// =====================================================================================================
+namespace {
+
+// H of m frames: every (frame, sub-frame) pair is one job; H = xor of the sub-frame digests.
+void hash_frames(vcrypt_ctx *c, const uint8_t *frames, size_t m, uint8_t *hashes) {
+    const uint32_t n = c->p.n_workers, h = c->g.h;
+    const size_t rb = c->g.row_bytes, fb = c->g.frame_bytes;
+    uint8_t *sub = c->subhash.data();
+    const bool simd = c->simd;
+    c->pool->parallel_for(m * n, [&](size_t job) {
+        const size_t f = job / n;
+        const uint32_t k = (uint32_t)(job - f * n);
+        const size_t r0 = vh::band_row(k, n, h), r1 = vh::band_row(k + 1, n, h);
+        vh::sha256(frames + f * fb + r0 * rb, (r1 - r0) * rb, sub + job * 32u, simd);
+    });
+    for (size_t f = 0; f < m; ++f) {
+        uint8_t *H = hashes + 32u * f;
+        std::memset(H, 0, 32);
+        for (uint32_t k = 0; k < n; ++k)
+            for (int b = 0; b < 32; ++b) H[b] ^= sub[(f * n + k) * 32u + b];
+    }
+}
+
+// D and B of m frames whose hashes are known, written frame after frame into D / B.  S is advanced.
+// Returns VCRYPT_E_STATE if a chaotic state became non-finite.
+int derive_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, uint16_t *D, uint8_t *B) {
+    const uint32_t n = c->p.n_workers;
+    const double gamma = c->p.gamma;
+    // the chain is serial in the frame index, and cheap (2n * K_m RK4 steps per frame)
+    for (size_t f = 0; f < m; ++f) {
+        double *IR = c->IR.data() + f * 2u * n * 4u;
+        if (!vh::chain_step(S, gamma, n, hashes + 32u * f, IR)) return VCRYPT_E_STATE;
+        vh::make_slices(IR, n, c->g.w, c->g.h, D + f * c->g.nD, B + f * c->g.frame_bytes, c->slices.data() + f * n);
+    }
+    const int isa = c->isa;
+    const size_t lanes = isa == 2 ? 8 : isa == 1 ? 4 : 1;
+    const size_t groups = (n + lanes - 1) / lanes;
+    std::atomic<bool> ok{true};
+    const vh::WorkerSlice *sl = c->slices.data();
+    c->pool->parallel_for(m * groups, [&](size_t job) {
+        const size_t f = job / groups, g0 = (job - f * groups) * lanes;
+        const size_t cnt = n - g0 < lanes ? n - g0 : lanes;
+        if (!vh::derive_workers(sl + f * n + g0, cnt, gamma, isa)) ok.store(false, std::memory_order_relaxed);
+    });
+    return ok.load() ? VCRYPT_OK : VCRYPT_E_STATE;
+}
+
+}  // namespace
+
+extern "C" int vcrypt_frame_hash(vcrypt_ctx *c, const uint8_t *frame, uint8_t *H_out) {
+    if (!c || !frame || !H_out) return VCRYPT_E_ARG;
+    hash_frames(c, frame, 1, H_out);
+    return VCRYPT_OK;
+}
+
+extern "C" int vcrypt_derive(vcrypt_ctx *c, const uint8_t *hash, uint16_t *D_out, uint8_t *B_out) {
+    if (!c || !hash || !D_out || !B_out) return VCRYPT_E_ARG;
+    double S[4];
+    std::memcpy(S, c->S, sizeof S);
+    const int rc = derive_frames(c, S, hash, 1, D_out, B_out);
+    if (rc != VCRYPT_OK) return rc;
+    std::memcpy(c->S, S, sizeof S);
+    c->frames_done += 1;
+    return VCRYPT_OK;
+}
+
+// =====================================================================================================
+// kernel-only path
+// =====================================================================================================
+static int device_call(vcrypt_ctx *c, bool decrypt, const void *d_in, const void *d_D, const void *d_B, size_t n,
+                       void *d_out, void *stream) {
+    if (!c || !d_in || !d_D || !d_B || !d_out) return VCRYPT_E_ARG;
+    if (!c->cuda) return VCRYPT_E_CUDA;
+    if ((((uintptr_t)d_in) | ((uintptr_t)d_out) | ((uintptr_t)d_B)) & 15u) return VCRYPT_E_ARG;
+    if (((uintptr_t)d_D) & 1u) return VCRYPT_E_ARG;
+    c->launches_last = 0;
+    if (n == 0) return VCRYPT_OK;
+    const uint8_t *a = static_cast<const uint8_t *>(d_in);
+    uint8_t *o = static_cast<uint8_t *>(d_out);
+    const size_t bytes = n * c->g.frame_bytes;
+    if (a != o && a < o + bytes && o < a + bytes) return VCRYPT_E_ARG;  // partial overlap
+    VC_CUDA(c, cudaSetDevice(c->device));
+    return launch_cipher(c, decrypt, a, static_cast<const uint16_t *>(d_D), static_cast<const uint8_t *>(d_B), n, o,
+                         static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int vcrypt_encrypt_device(vcrypt_ctx *c, const void *d_frames, const void *d_D, const void *d_B, size_t n,
+                                     void *d_cipher, void *stream) {
+    return device_call(c, false, d_frames, d_D, d_B, n, d_cipher, stream);
+}
+
+extern "C" int vcrypt_decrypt_device(vcrypt_ctx *c, const void *d_cipher, const void *d_D, const void *d_B, size_t n,
+                                     void *d_plain, void *stream) {
+    return device_call(c, true, d_cipher, d_D, d_B, n, d_plain, stream);
+}
+
+// =====================================================================================================
+// host-buffer pipeline: Algorithm 1's loop over frames, batched and overlapped
+// =====================================================================================================
+static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint8_t *hashes_in, size_t n, uint8_t *out,
+                      uint8_t *hashes_out) {
+    if (!c || !in || !out || (decrypt ? !hashes_in : !hashes_out)) return VCRYPT_E_ARG;
+    if (!c->cuda) return VCRYPT_E_CUDA;
+    c->launches_last = 0;
+    for (double &v : c->stage_ms) v = 0.0;
+    if (n == 0) return VCRYPT_OK;
+    VC_CUDA(c, cudaSetDevice(c->device));
+    const size_t fb = c->g.frame_bytes, nD = c->g.nD;
+    const bool in_pinned = is_pinned(in) && is_pinned(in + n * fb - 1);
+    const bool out_pinned = is_pinned(out) && is_pinned(out + n * fb - 1);
+    const bool generic = !c->plan.tiled || (c->p.flags & VCRYPT_FLAG_FORCE_GENERIC);
+    double S[4];
+    std::memcpy(S, c->S, sizeof S);
+    int rc = VCRYPT_OK;
+    size_t k = 0;
+    for (size_t b0 = 0; b0 < n && rc == VCRYPT_OK; b0 += c->batch, ++k) {
+        const size_t m = n - b0 < c->batch ? n - b0 : c->batch;
+        Slot &s = c->slots[k % c->slots.size()];
+        if ((rc = retire_slot(c, s)) != VCRYPT_OK) break;
+        if ((rc = ensure_slot(c, s, !in_pinned, !out_pinned)) != VCRYPT_OK) break;
+        const uint8_t *src = in + b0 * fb;
+        const uint8_t *hs = hashes_in ? hashes_in + 32u * b0 : nullptr;
+        if (!decrypt) {  // Algorithm 1 steps 4-6
+            const auto t0 = clk::now();
+            hash_frames(c, src, m, hashes_out + 32u * b0);
+            hs = hashes_out + 32u * b0;
+            c->stage_ms[0] += ms_since(t0);
+        }
+        {  // steps 7-14
+            const auto t0 = clk::now();
+            rc = derive_frames(c, S, hs, m, s.h_D, s.h_B);
+            c->stage_ms[1] += ms_since(t0);
+            if (rc != VCRYPT_OK) break;
+        }
+        if (!in_pinned) {
+            const auto t0 = clk::now();
+            const size_t chunk = (size_t)1 << 20, total = m * fb, nch = (total + chunk - 1) / chunk;
+            uint8_t *dst = s.h_F;
+            c->pool->parallel_for(nch, [&](size_t i) {
+                const size_t o = i * chunk, len = total - o < chunk ? total - o : chunk;
+                std::memcpy(dst + o, src + o, len);
+            });
+            c->stage_ms[2] += ms_since(t0);
+        }
+        // steps 15-21: upload, GPU steps, download -- asynchronous on the slot's stream
+        uint8_t *d_res = generic ? s.d_out : s.d_F;
+        uint8_t *h_res = out_pinned ? out + b0 * fb : s.h_out;
+        cudaError_t e = cudaMemcpyAsync(s.d_F, in_pinned ? src : s.h_F, m * fb, cudaMemcpyHostToDevice, s.st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(s.d_D, s.h_D, m * nD * sizeof(uint16_t), cudaMemcpyHostToDevice, s.st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(s.d_B, s.h_B, m * fb, cudaMemcpyHostToDevice, s.st);
+        if (e != cudaSuccess) { rc = cuda_fail(c, e, "upload"); break; }
+        if ((rc = launch_cipher(c, decrypt, s.d_F, s.d_D, s.d_B, m, d_res, s.st)) != VCRYPT_OK) break;
+        e = cudaMemcpyAsync(h_res, d_res, m * fb, cudaMemcpyDeviceToHost, s.st);
+        if (e == cudaSuccess) e = cudaEventRecord(s.done, s.st);
+        if (e != cudaSuccess) { rc = cuda_fail(c, e, "download"); break; }
+        s.busy = true;
+        s.user_out = out_pinned ? nullptr : out + b0 * fb;
+        s.out_bytes = m * fb;
+    }
+    // drain in submission order
+    for (size_t i = 0; i < c->slots.size(); ++i) {
+        Slot &s = c->slots[(k + i) % c->slots.size()];
+        const int r2 = retire_slot(c, s);
+        if (rc == VCRYPT_OK) rc = r2;
+    }
+    if (rc != VCRYPT_OK) return rc;  // chain untouched
+    std::memcpy(c->S, S, sizeof S);
+    c->frames_done += n;
+    return VCRYPT_OK;
+}
+
+extern "C" int vcrypt_encrypt_frames(vcrypt_ctx *c, const uint8_t *frames, size_t n, uint8_t *cipher_out,
+                                     uint8_t *hashes_out) {
+    return run_frames(c, false, frames, nullptr, n, cipher_out, hashes_out);
+}
+
+extern "C" int vcrypt_decrypt_frames(vcrypt_ctx *c, const uint8_t *cipher, const uint8_t *hashes, size_t n,
+                                     uint8_t *plain_out) {
+    return run_frames(c, true, cipher, hashes, n, plain_out, nullptr);
+}
