@@ -1,0 +1,243 @@
+"""GPU parity (run with -m gpu on the B200 box): the CUDA path, called through the C ABI, against the CPU
+oracle, bit for bit (integer / byte work: the bar is exact equality).
+
+Kernel level  : vcrypt_encrypt_device / vcrypt_decrypt_device with random D, B (rows a6-a10, a12) against the
+                oracle's literal bit-matrix Algorithms 3-7, over tiled shapes, ragged any-shape cases, special
+                distances and in-place calls.
+Whole path    : vcrypt_encrypt_frames / vcrypt_decrypt_frames (rows a1-a12) against the oracle's Algorithm 1
+                on the BASELINE.json configs: C1, C2 in full element by element; C3-C5 at full size in bench's
+                launch configuration with every hash compared, sampled frames compared element by element
+                and the round trip checked on every frame.
+"""
+import numpy as np
+import pytest
+
+from paper_2505_07158_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+
+    assert torch.cuda.is_available(), "these tests need the B200"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def vb():
+    from paper_2505_07158_b200 import binding
+
+    return binding
+
+
+def gpu_ctx(vb, w, h, n=synth.N_WORKERS, **kw):
+    return vb.Vcrypt(synth.KEY, synth.GAMMA, n, w, h, **kw)
+
+
+def run_device(torch, v, F, D, B, decrypt=False, inplace=False):
+    dF = torch.from_numpy(F).cuda()
+    dD = torch.from_numpy(D.view(np.int16)).cuda()
+    dB = torch.from_numpy(B).cuda()
+    dO = dF if inplace else torch.empty_like(dF)
+    (v.decrypt_device if decrypt else v.encrypt_device)(dF, dD, dB, dO)
+    torch.cuda.synchronize()
+    return dO.cpu().numpy()
+
+
+def rnd_case(w, h, nf, seed, dmode="random"):
+    rng = np.random.default_rng(seed)
+    F = rng.integers(0, 256, (nf, h, w, 3), dtype=np.uint8)
+    B = rng.integers(0, 256, (nf, h, w, 3), dtype=np.uint8)
+    nD = 3 * (h + w)
+    if dmode == "random":
+        D = rng.integers(0, 65536, (nf, nD), dtype=np.uint16)
+    elif dmode == "zero":
+        D = np.zeros((nf, nD), np.uint16)
+    elif dmode == "max":
+        D = np.full((nf, nD), 65535, np.uint16)
+    elif dmode == "bytes":  # horizontal distances multiples of 8: pure byte rolls
+        D = (rng.integers(0, 8192, (nf, nD)) * 8).astype(np.uint16)
+    elif dmode == "wrap":  # distances at the modulus boundaries
+        D = rng.choice(np.array([0, 1, 7, 8, 8 * w - 1, 8 * w, 8 * w + 1, h - 1, h, h + 1, 31, 32, 33], np.int64) % 65536,
+                       (nf, nD)).astype(np.uint16)
+    return F, D, B
+
+
+def oracle_frames(orc, F, D, B, inverse=False):
+    return np.stack([orc.confuse_xor(F[k], D[k], B[k], inverse=inverse) for k in range(F.shape[0])])
+
+
+# shapes on the tiled path (w % 16 == 0): several column strips, ragged last strip, several row blocks
+TILED = [(256, 256, 1), (64, 48, 3), (16, 1, 2), (16, 5, 1), (48, 33, 2), (640, 480, 2), (80, 7, 4), (1008, 19, 1)]
+# shapes only the any-shape kernels take
+RAGGED = [(1, 1, 1), (1, 7, 2), (5, 1, 1), (17, 9, 3), (33, 20, 2), (100, 37, 1), (15, 64, 1), (250, 3, 2)]
+
+
+@pytest.mark.parametrize("w,h,nf", TILED + RAGGED)
+@pytest.mark.parametrize("dmode", ["random", "wrap"])
+def test_kernels_match_oracle(torch_cuda, vb, orc, w, h, nf, dmode):
+    F, D, B = rnd_case(w, h, nf, seed=w * 131 + h * 7 + nf, dmode=dmode)
+    v = gpu_ctx(vb, w, h)
+    E = run_device(torch_cuda, v, F, D, B)
+    assert np.array_equal(E, oracle_frames(orc, F, D, B))
+    assert v.launch_count()[0] >= 1
+    P = run_device(torch_cuda, v, E, D, B, decrypt=True)
+    assert np.array_equal(P, oracle_frames(orc, E, D, B, inverse=True))
+    assert np.array_equal(P, F)
+
+
+@pytest.mark.parametrize("dmode", ["zero", "max", "bytes"])
+@pytest.mark.parametrize("w,h", [(64, 48), (17, 9), (256, 64)])
+def test_special_distances(torch_cuda, vb, orc, w, h, dmode):
+    F, D, B = rnd_case(w, h, 2, seed=5, dmode=dmode)
+    v = gpu_ctx(vb, w, h)
+    E = run_device(torch_cuda, v, F, D, B)
+    assert np.array_equal(E, oracle_frames(orc, F, D, B))
+    if dmode == "zero":
+        assert np.array_equal(E, F ^ B)  # identity confusion: Algorithm 6 alone
+    assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
+
+
+@pytest.mark.parametrize("w,h,nf", [(64, 48, 3), (256, 256, 2), (17, 9, 2)])
+@pytest.mark.parametrize("generic", [False, True])
+def test_in_place_and_forced_generic(torch_cuda, vb, orc, w, h, nf, generic):
+    F, D, B = rnd_case(w, h, nf, seed=11)
+    v = gpu_ctx(vb, w, h, flags=vb.FLAG_FORCE_GENERIC if generic else 0)
+    ref = oracle_frames(orc, F, D, B)
+    assert np.array_equal(run_device(torch_cuda, v, F, D, B), ref)
+    assert np.array_equal(run_device(torch_cuda, v, F, D, B, inplace=True), ref)
+    assert np.array_equal(run_device(torch_cuda, v, ref, D, B, decrypt=True, inplace=True), F)
+
+
+def test_many_frames_per_call_split_into_l2_sized_launches(torch_cuda, vb, orc):
+    """More frames than one L2-resident launch holds: the call splits, results unchanged."""
+    w, h, nf = 640, 480, 80  # 73.7 MB of frames
+    F, D, B = rnd_case(w, h, nf, seed=21)
+    v = gpu_ctx(vb, w, h)
+    E = run_device(torch_cuda, v, F, D, B)
+    for k in (0, 1, 37, 68, 69, 70, 79):
+        assert np.array_equal(E[k], orc.confuse_xor(F[k], D[k], B[k])), k
+    assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
+
+
+def test_device_call_argument_errors(torch_cuda, vb):
+    torch = torch_cuda
+    v = gpu_ctx(vb, 64, 48)
+    F, D, B = rnd_case(64, 48, 2, seed=1)
+    dF, dD, dB = torch.from_numpy(F).cuda(), torch.from_numpy(D.view(np.int16)).cuda(), torch.from_numpy(B).cuda()
+    L = v.L
+    st = torch.cuda.current_stream().cuda_stream
+    assert L.vcrypt_encrypt_device(v._p, None, dD.data_ptr(), dB.data_ptr(), 2, dF.data_ptr(), st) == vb.E_ARG
+    assert L.vcrypt_encrypt_device(v._p, dF.data_ptr() + 1, dD.data_ptr(), dB.data_ptr(), 1, dF.data_ptr(), st) == vb.E_ARG
+    # partial overlap of input and output
+    assert L.vcrypt_encrypt_device(v._p, dF.data_ptr(), dD.data_ptr(), dB.data_ptr(), 2, dF.data_ptr() + 64 * 48 * 3, st) == vb.E_ARG
+    assert L.vcrypt_encrypt_device(v._p, dF.data_ptr(), dD.data_ptr(), dB.data_ptr(), 0, dF.data_ptr(), st) == vb.OK
+
+
+# ------------------------------------------------------------------------------------------------------
+# whole path
+# ------------------------------------------------------------------------------------------------------
+def test_config1_full(vb, orc):
+    cfg = synth.CONFIGS["C1"]
+    frames = synth.video(cfg)
+    assert synth.digest(frames) == synth.digest(synth.video(cfg))  # generator is deterministic
+    enc = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch)
+    C, Hs = enc.encrypt_frames(frames)
+    oc = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    Co, Ho = oc.encrypt_frames(frames)
+    assert np.array_equal(Hs, Ho)
+    assert np.array_equal(C, Co)
+    dec = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch)
+    assert np.array_equal(dec.decrypt_frames(C, Hs), frames)
+
+
+def test_config2_full(vb, orc):
+    cfg = synth.CONFIGS["C2"]
+    frames = synth.video(cfg)
+    enc = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
+    C, Hs = enc.encrypt_frames(frames)
+    oc = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    Co, Ho = oc.encrypt_frames(frames)
+    assert np.array_equal(Hs, Ho)
+    assert np.array_equal(C, Co)
+    od = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    dec = gpu_ctx(vb, cfg.w, cfg.h, batch=5, n_streams=2)  # another pipeline shape: results must not change
+    P = dec.decrypt_frames(C, Hs)
+    assert np.array_equal(P, od.decrypt_frames(Co, Ho))
+    assert np.array_equal(P, frames)
+
+
+def sampled_parity(vb, orc, cfg, nframes, sample, pinned):
+    """Full-size config in bench's launch configuration: all hashes, sampled frames element by element
+    (oracle D, B follow the whole chain), round trip on every frame."""
+    import torch
+
+    if pinned:
+        tin = torch.empty((nframes, cfg.h, cfg.w, 3), dtype=torch.uint8).pin_memory()
+        frames = synth.video(cfg, nframes, out=tin.numpy())
+        tout = torch.empty_like(tin).pin_memory()
+        C = tout.numpy()
+    else:
+        frames = synth.video(cfg, nframes)
+        C = np.empty_like(frames)
+    Hs = np.empty((nframes, 32), np.uint8)
+    enc = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
+    enc.encrypt_frames(frames, C, Hs)
+    oc = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    for k in range(nframes):
+        H = orc.frame_hash(frames[k], synth.N_WORKERS)
+        assert H == Hs[k].tobytes(), k
+        D, B = oc.derive(H)
+        if k in sample:
+            assert np.array_equal(C[k], orc.confuse_xor(frames[k], D, B)), k
+    dec = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
+    P = dec.decrypt_frames(C, Hs)
+    assert np.array_equal(P, frames)
+    return enc
+
+
+def test_config3_fhd_batch1(vb, orc):
+    cfg = synth.CONFIGS["C3"]
+    sampled_parity(vb, orc, cfg, cfg.frames, {0, 1, 2, 15, 29}, pinned=False)
+
+
+def test_config4_fhd_batches_of_8_three_streams(vb, orc):
+    cfg = synth.CONFIGS["C4"]
+    enc = sampled_parity(vb, orc, cfg, 100, {0, 7, 8, 9, 50, 95, 96, 99}, pinned=True)  # 12 full batches + 4
+    assert enc.launch_count()[1] >= 13
+
+
+def test_config5_4k(vb, orc):
+    cfg = synth.CONFIGS["C5"]
+    sampled_parity(vb, orc, cfg, 20, {0, 7, 8, 19}, pinned=True)
+
+
+def test_config4_one_bit_pairs_npcr_uaci(vb):
+    """Pin P7 on the GPU path: one flipped plaintext bit -> NPCR ~ 255/256, UACI ~ (256^2-1)/(3*256*255)
+    (Eq. 14-16; closed forms for independent uniform ciphertexts)."""
+    cfg = synth.CONFIGS["C4"]
+    npcr, uaci = [], []
+    for f, g, _ in synth.one_bit_pairs(cfg, 6):
+        c1, _ = gpu_ctx(vb, cfg.w, cfg.h, batch=1).encrypt_frames(f[None])
+        c2, _ = gpu_ctx(vb, cfg.w, cfg.h, batch=1).encrypt_frames(g[None])
+        a, b = c1[0].astype(np.int16), c2[0].astype(np.int16)
+        npcr.append(100.0 * np.mean(a != b))
+        uaci.append(100.0 * np.mean(np.abs(a - b)) / 255.0)
+    n = 3 * cfg.w * cfg.h
+    s_npcr = 100.0 * np.sqrt((255 / 256) * (1 / 256) / n)
+    assert all(abs(x - 99.609375) < 5 * s_npcr for x in npcr), npcr
+    assert all(abs(x - 33.463542) < 5 * 0.0095 for x in uaci), uaci
+
+
+def test_failed_call_leaves_chain_untouched(vb):
+    v = gpu_ctx(vb, 64, 48)
+    s0 = v.get_state()
+    f = synth.random_frames(64, 48, 2, 1)
+    rc = v.L.vcrypt_encrypt_frames(v._p, f.ctypes.data, 2, None, None)
+    assert rc == vb.E_ARG
+    s1 = v.get_state()
+    assert s0[1] == s1[1] and np.array_equal(s0[0], s1[0])
+    v.encrypt_frames(f)
+    assert v.get_state()[1] == 2
