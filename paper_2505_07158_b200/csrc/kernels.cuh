@@ -23,13 +23,14 @@ inline Geom make_geom(uint32_t w, uint32_t h) {
 
 // Plan chosen once per context from (w, h) and the device's shared-memory size.
 struct Plan {
-    bool tiled;            // tiled two-pass path usable (w % 16 == 0 and a column strip fits in shared memory)
-    int strip_bytes;       // X: byte-columns per strip (128 / 64 / 32 / 16)
+    bool tiled;            // tiled two-pass path usable (w % 16 == 0, h % 4 == 0, h >= 16, strip and row block fit in shared memory)
+    int strip_bytes;       // X: byte columns per strip (128, 64 or 32)
     int strips_per_frame;  // ceil(3w / X)
-    int rows_per_block;    // row pass: rows a CTA stages at once
+    int row_threads;       // row pass: threads per CTA
+    int row_grid_max;      // row pass: persistent CTAs (resident CTAs per SM x SMs)
+    int col_ctas_per_sm;   // residency the column pass was sized for (3: 256-thread CTAs, 1: 512-thread CTAs)
     size_t smem_row;       // dynamic shared memory of the row pass
     size_t smem_col;       // dynamic shared memory of the column pass
-    int col_ctas_per_sm;   // residency the column pass was sized for
     size_t max_frames_per_launch;  // keeps the intermediate (n * 3wh bytes) L2-resident
 };
 
