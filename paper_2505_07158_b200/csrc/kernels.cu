@@ -33,6 +33,8 @@
 //
 // A one-thread-per-output-byte gather kernel covers every shape the tiled passes do not
 // (w % 16 != 0, h % 4 != 0, h < 16, or a strip / row block too large for shared memory).
+#include <cuda.h>
+
 #include "kernels.cuh"
 
 namespace vk {
@@ -174,148 +176,431 @@ __device__ __forceinline__ uint32_t gather4(const uint32_t *r, int i0, int b0, i
 // ---------------------------------------------------------------------------------------------
 // Row pass: horizontal bit rotation (Algorithm 4 / Eq. 2 on the rows of Algorithm 3's bit matrix,
 // packed back as in Algorithm 7).  Work unit = one block of 4 consecutive rows of one frame (h % 4 == 0,
-// so a block never straddles two frames); one item = 16 pixels (48 bytes) of each of the 4 rows.
+// so a block never straddles two frames).
 //   INV = false: bit p of channel c moves to (p + d_h mod 8w) mod 8w; the block is written in T4 layout.
 //   INV = true : the inverse rotation; input and output are row-major.
-// Persistent CTAs walk the blocks round-robin with a three-buffer ring: while block i is being rotated,
-// the bulk async load (TMA, cp.async.bulk) of blocks i+1 and i+2 and the bulk store of block i-1 are in
-// flight.  A buffer is: loaded -> de-interleaved into planes -> overwritten with the rotated block ->
-// stored.  A plane (one row, one channel: w/4 words) is kept as chunks of 4 words at a stride of 5 words
-// (odd: thread k's chunk sits at bank 5k + i, no conflicts), plus a copy of chunk 0 at the end so that the
-// 5-word window of a funnel shift never wraps.
+// Warp-specialised persistent CTAs.  The last warp is the copy warp: it computes the shift parameters of
+// a block from D, brings the block into a ring of NS shared-memory stages with one bulk async copy (TMA,
+// cp.async.bulk -> UBLKCP), and sends finished blocks back with one bulk async store.  The other
+// NC threads are compute threads and work on a stage in two phases separated by a named barrier:
+//   phase 1 (one item = 16 pixels of one row): 48 interleaved bytes -> three channel planes (PRMT network),
+//            so that the per-(row, channel) bit rotation becomes a 32-bit funnel shift of two neighbouring
+//            plane words; the chunk is stored already rotated by the whole-chunk part of the distance;
+//   phase 2 (one item = a quad of 4 pixels, all 4 rows, all 3 channels): 12 funnel shifts, then either three
+//            4 x 4 byte transposes (T4: the word at (row 4R + (x & 3), word column x >> 2) holds byte column x
+//            of rows 4R .. 4R+3) or the re-interleave to row-major; the result overwrites the stage.
+// Synchronisation: full[s] (mbarrier, transaction bytes) copy warp -> compute threads; done[s] (mbarrier,
+// one arrival) compute threads -> copy warp; named barrier 1 among the compute threads.
 // In place (dst == src) is safe: a block is read completely before it is written.
 // ---------------------------------------------------------------------------------------------
-constexpr int ROW_RB = 4;      // rows per block
-constexpr int ROW_HDR = 256;   // 3 mbarriers + 2 x 12 shift parameters
-constexpr int ROW_NBUF = 3;
+constexpr int ROW_RB = 4;       // rows per block
+constexpr int ROW_HDR = 1024;   // mbarriers + shift parameters
+constexpr int ROW_MAXNS = 4;    // stages at most
 
-// shift parameter of one (row, channel): bits 0-4 bit shift, 8-9 first slot, 16-31 chunk shift
-__device__ __forceinline__ uint32_t row_param(const uint16_t *__restrict__ D, const Geom &g, uint32_t grow, uint32_t ch,
-                                              bool inv) {
+// Rotation of one (row, channel): output bit d takes source bit (d + sh) mod 8w, sh = 32 * (4 * dq + fine) + sh5.
+// Phase 1 writes chunk k (16 pixels) of the plane at chunk position (k - dq) mod C, so that phase 2 reads the two
+// words q + fine, q + fine + 1 of the pre-rotated plane (never wrapping: two pad chunks repeat chunks 0 and 1).
+//   p1 = 16 * dq                      (bytes; phase 1)
+//   p2 = (plane offset + 4 * fine) << 8 | sh5   (phase 2: one LEA.HI gives the address, the funnel shift takes sh5)
+__device__ __forceinline__ uint2 row_param(const uint16_t *__restrict__ D, const Geom &g, uint32_t grow, uint32_t ch,
+                                           bool inv, uint32_t plane_off) {
     const uint32_t f = grow / g.h, i = grow - f * g.h, W8 = 8u * g.w;
     const uint32_t s = (uint32_t)D[(size_t)f * g.nD + ch * (g.h + g.w) + i] % W8;
-    const uint32_t sh = inv ? s : (s ? W8 - s : 0u);  // output bit d takes source bit (d + sh) mod 8w
-    const uint32_t dw = sh >> 5;                      // source word offset
-    return (sh & 31u) | ((dw & 3u) << 8) | ((dw >> 2) << 16);
+    const uint32_t sh = inv ? s : (s ? W8 - s : 0u);
+    const uint32_t dw = sh >> 5;
+    return make_uint2((dw >> 2) << 4, ((plane_off + 4u * (dw & 3u)) << 8) | (sh & 31u));
 }
 
-template <bool INV>
-__global__ void __launch_bounds__(256) row_pass_kernel(const uint8_t *src, uint8_t *dst, const uint16_t *__restrict__ D,
-                                                       Geom g, uint32_t nblocks) {
+__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void bulk_g2s_hint(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(__cvta_generic_to_global(gsrc)), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_hint(void *gdst, const void *smem_src, uint32_t bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(
+                     __cvta_generic_to_global(gdst)),
+                 "r"(smem_u32(smem_src)), "r"(bytes), "l"(pol)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read_0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
+template <bool INV, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src, uint8_t *dst, const uint16_t *__restrict__ D,
+                                                           Geom g, uint32_t nblocks, uint32_t NS, uint32_t NC) {
     extern __shared__ __align__(128) uint8_t smem[];
-    uint64_t *bar = reinterpret_cast<uint64_t *>(smem);           // [ROW_NBUF]
-    uint32_t *par = reinterpret_cast<uint32_t *>(smem + 64);      // [2][16]
-    const uint32_t w = g.w, rb = g.row_bytes, C = w >> 4;          // C items per row
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);                // [ROW_MAXNS]
+    uint64_t *done = reinterpret_cast<uint64_t *>(smem + 64);           // [ROW_MAXNS]
+    uint32_t *par1 = reinterpret_cast<uint32_t *>(smem + 128);          // [ROW_MAXNS][4 rows][4]  (64 B per stage)
+    uint32_t *par2 = reinterpret_cast<uint32_t *>(smem + 128 + 64 * ROW_MAXNS);  // same shape
+    const uint32_t w = g.w, rb = g.row_bytes, C = w >> 4, Q = w >> 2;   // items / quads per row
     const uint32_t blk_bytes = ROW_RB * rb;
-    const uint32_t plane_stride = 20u * (C + 1u);                  // bytes: (C + 1) chunks of 5 words
+    const uint32_t PS = w + 32u;                                        // plane stride (bytes): w/4 words + 2 pad chunks
     uint8_t *stage0 = smem + ROW_HDR;
-    uint8_t *planes = stage0 + ROW_NBUF * blk_bytes;
+    uint8_t *planes = stage0 + NS * blk_bytes;
     const uint32_t G = gridDim.x, tid = threadIdx.x;
+    const uint32_t blk0 = blockIdx.x;
+    if (blk0 >= nblocks) return;
+    const uint32_t niter = (nblocks - blk0 + G - 1) / G;
 
-    uint32_t blk = blockIdx.x;
-    if (blk >= nblocks) return;
     if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < ROW_NBUF; ++s) mbar_init(bar + s, 1);
-        mbar_expect_tx(bar + 0, blk_bytes);
-        bulk_g2s(stage0, src + (size_t)blk * blk_bytes, blk_bytes, bar + 0);
-        if (blk + G < nblocks) {
-            mbar_expect_tx(bar + 1, blk_bytes);
-            bulk_g2s(stage0 + blk_bytes, src + (size_t)(blk + G) * blk_bytes, blk_bytes, bar + 1);
-        }
+        for (uint32_t s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(done + s, 1); }
     }
-    if (tid < 3 * ROW_RB) par[tid] = row_param(D, g, blk * ROW_RB + tid / 3u, tid % 3u, INV);
-    __syncthreads();  // mbarriers initialised, parameters of the first block visible
+    __syncthreads();
 
-    uint32_t s = 0;
-    for (uint32_t it = 0; blk < nblocks; ++it, blk += G) {
+    if (tid >= NC) {
+        // ================= copy warp =================
+        const uint32_t lane = tid - NC;
+        const uint32_t pr = lane / 3u, pch = lane - 3u * pr;           // lanes 0..11: (row, channel) of the block
+        const uint32_t pslot = pr * 4u + pch, poff = (pr * 3u + pch) * PS;
+        const uint64_t pol_in = policy_evict_first();
+        // prologue: fill every stage
+        for (uint32_t it = 0; it < NS && it < niter; ++it) {
+            const uint32_t blk = blk0 + it * G;
+            if (lane < 3 * ROW_RB) {
+                const uint2 pv = row_param(D, g, blk * ROW_RB + pr, pch, INV, poff);
+                par1[it * 16u + pslot] = pv.x;
+                par2[it * 16u + pslot] = pv.y;
+            }
+            __syncwarp();
+            if (lane == 0) {
+                mbar_expect_tx(full + it, blk_bytes);
+                bulk_g2s_hint(stage0 + it * blk_bytes, src + (size_t)blk * blk_bytes, blk_bytes, full + it, pol_in);
+            }
+        }
+        uint32_t s = 0, ph = 0;
+        for (uint32_t it = 0; it < niter; ++it) {
+            const uint32_t blk = blk0 + it * G;
+            const bool refill = it + NS < niter;
+            uint2 pnext = make_uint2(0u, 0u);
+            if (refill && lane < 3 * ROW_RB) pnext = row_param(D, g, (blk + NS * G) * ROW_RB + pr, pch, INV, poff);
+            if (lane == 0) {
+                mbar_wait(done + s, ph);  // the compute threads have written block `it` back into the stage
+                bulk_s2g(dst + (size_t)blk * blk_bytes, stage0 + s * blk_bytes, blk_bytes);
+            }
+            __syncwarp();
+            if (refill) {
+                if (lane < 3 * ROW_RB) { par1[s * 16u + pslot] = pnext.x; par2[s * 16u + pslot] = pnext.y; }
+                __syncwarp();
+                if (lane == 0) {
+                    bulk_wait_read_0();  // the store has left shared memory
+                    mbar_expect_tx(full + s, blk_bytes);
+                    bulk_g2s_hint(stage0 + s * blk_bytes, src + (size_t)(blk + NS * G) * blk_bytes, blk_bytes, full + s, pol_in);
+                }
+            }
+            if (++s == NS) { s = 0; ph ^= 1u; }
+        }
+        if (lane == 0) bulk_wait_all();
+        return;
+    }
+
+    // ================= compute threads =================
+    // loop-invariant work assignment: phase 1 item (row r1, chunk k1) = tid (further items: + NC), phase 2 quad = tid
+    const uint32_t r1 = (tid >= C) + (tid >= 2u * C) + (tid >= 3u * C), k1 = tid - r1 * C;
+    uint32_t s = 0, ph = 0;
+    for (uint32_t it = 0; it < niter; ++it) {
         uint8_t *stage = stage0 + s * blk_bytes;
-        const uint32_t *pc = par + (it & 1u) * 16u;
-        uint32_t pnext = 0;
-        if (tid < 3 * ROW_RB && blk + G < nblocks) pnext = row_param(D, g, (blk + G) * ROW_RB + tid / 3u, tid % 3u, INV);
-        mbar_wait(bar + s, (it / ROW_NBUF) & 1u);
+        const uint32_t *p1 = par1 + s * 16u, *p2 = par2 + s * 16u;
+        mbar_wait(full + s, ph);
 
-        // ---- de-interleave into planes
-        for (uint32_t k = tid; k < C; k += blockDim.x) {
+        // ---- phase 1: de-interleave into planes; item = (row r, 16 pixels k)
+        for (uint32_t i = tid; i < ROW_RB * C; i += NC) {
+            uint32_t r = r1, k = k1;
+            if (i != tid) { r = (i >= C) + (i >= 2u * C) + (i >= 3u * C); k = i - r * C; }
+            const uint4 *p = reinterpret_cast<const uint4 *>(stage + r * rb + 48u * k);
+            const uint4 a = p[0], b = p[1], c = p[2];
+            const uint4 dq = *reinterpret_cast<const uint4 *>(p1 + 4u * r);
+            const uint32_t W[12] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c.x, c.y, c.z, c.w};
+            uint4 v0, v1, v2;  // channel 0, 1, 2: four plane words each
+#define VK_DEINT(m, X0, X1, X2)                                                     \
+    X0 = __byte_perm(__byte_perm(W[3 * m], W[3 * m + 1], 0x0630), W[3 * m + 2], 0x5210); \
+    X1 = __byte_perm(__byte_perm(W[3 * m], W[3 * m + 1], 0x0741), W[3 * m + 2], 0x6210); \
+    X2 = __byte_perm(__byte_perm(W[3 * m], W[3 * m + 1], 0x0052), W[3 * m + 2], 0x7410);
+            VK_DEINT(0, v0.x, v1.x, v2.x)
+            VK_DEINT(1, v0.y, v1.y, v2.y)
+            VK_DEINT(2, v0.z, v1.z, v2.z)
+            VK_DEINT(3, v0.w, v1.w, v2.w)
+#undef VK_DEINT
+            uint8_t *pl = planes + r * 3u * PS;
+            const int32_t k16 = (int32_t)(16u * k);
+#define VK_PUT(V, DQ, CH)                                                      \
+    {                                                                          \
+        int32_t kb = k16 - (int32_t)(DQ);                                      \
+        if (kb < 0) kb += (int32_t)w;                                          \
+        uint8_t *d = pl + (CH) * PS + kb;                                      \
+        *reinterpret_cast<uint4 *>(d) = V;                                     \
+        if (kb < 32) *reinterpret_cast<uint4 *>(d + w) = V; /* pad chunks */   \
+    }
+            VK_PUT(v0, dq.x, 0u)
+            VK_PUT(v1, dq.y, 1u)
+            VK_PUT(v2, dq.z, 2u)
+#undef VK_PUT
+        }
+        named_bar_sync(1, NC);  // planes complete; the raw block in `stage` may now be overwritten
+
+        // ---- phase 2: rotate; item = quad q (4 pixels) of all 4 rows and 3 channels
+        for (uint32_t q = tid; q < Q; q += NC) {
+            const uint8_t *qa = planes + 4u * q;
+            uint32_t R[ROW_RB][3];
 #pragma unroll
             for (int r = 0; r < ROW_RB; ++r) {
-                const uint4 *p = reinterpret_cast<const uint4 *>(stage + r * rb + 48u * k);
-                const uint4 a = p[0], b = p[1], c = p[2];
-                const uint32_t in[12] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c.x, c.y, c.z, c.w};
+                const uint4 pv = *reinterpret_cast<const uint4 *>(p2 + 4 * r);
+                const uint32_t pvv[3] = {pv.x, pv.y, pv.z};
 #pragma unroll
                 for (int ch = 0; ch < 3; ++ch) {
-                    uint32_t *pb = reinterpret_cast<uint32_t *>(planes + (r * 3 + ch) * plane_stride) + 5u * k;
-#pragma unroll
-                    for (int m = 0; m < 4; ++m) {
-                        const int o = 12 * m + ch;  // byte offsets o, o+3, o+6, o+9 of the 48
-                        const uint32_t v = gather4(in, o >> 2, o & 3, (o + 3) >> 2, (o + 3) & 3, (o + 6) >> 2, (o + 6) & 3,
-                                                   (o + 9) >> 2, (o + 9) & 3);
-                        pb[m] = v;
-                        if (k == 0) pb[5u * C + m] = v;
-                    }
+                    const uint32_t *P = reinterpret_cast<const uint32_t *>(qa + (pvv[ch] >> 8));
+                    R[r][ch] = __funnelshift_r(P[0], P[1], pvv[ch]);  // shift amount = low 5 bits
                 }
             }
-        }
-        __syncthreads();  // planes complete; the raw block in `stage` may now be overwritten
-
-        // ---- rotate, re-interleave, write the output block over the input block
-        for (uint32_t k = tid; k < C; k += blockDim.x) {
-            uint32_t R[ROW_RB * 3 * 4];  // [r][ch][word]
-#pragma unroll
-            for (int r = 0; r < ROW_RB; ++r)
+            uint8_t *o = stage + 12u * q;
+            if (!INV) {
+                // T4: pixel p of the quad, channel ch = byte column x = 12q + 3p + ch -> block row x & 3, word x >> 2
 #pragma unroll
                 for (int ch = 0; ch < 3; ++ch) {
-                    const uint32_t pv = pc[r * 3 + ch];
-                    const uint32_t slot0 = (pv >> 8) & 3u;
-                    uint32_t kb = k + (pv >> 16);
-                    if (kb >= C) kb -= C;
-                    const uint32_t *q = reinterpret_cast<const uint32_t *>(planes + (r * 3 + ch) * plane_stride) + 5u * kb + slot0;
-                    const uint32_t v0 = q[0], v1 = q[1], v2 = q[2], v3 = q[3], v4 = q[4], v5 = q[5];
-                    // the window skips the unused 5th word of a chunk after (4 - slot0) words
-                    const uint32_t w1 = slot0 == 3u ? v2 : v1, w2 = slot0 >= 2u ? v3 : v2, w3 = slot0 >= 1u ? v4 : v3;
-                    uint32_t *o = R + (r * 3 + ch) * 4;
-                    o[0] = __funnelshift_r(v0, w1, pv);  // shift amount = pv & 31
-                    o[1] = __funnelshift_r(w1, w2, pv);
-                    o[2] = __funnelshift_r(w2, w3, pv);
-                    o[3] = __funnelshift_r(w3, v5, pv);
-                }
+                    const uint32_t t01a = __byte_perm(R[0][ch], R[1][ch], 0x5140), t01b = __byte_perm(R[0][ch], R[1][ch], 0x7362);
+                    const uint32_t t23a = __byte_perm(R[2][ch], R[3][ch], 0x5140), t23b = __byte_perm(R[2][ch], R[3][ch], 0x7362);
+                    const uint32_t T[4] = {__byte_perm(t01a, t23a, 0x5410), __byte_perm(t01a, t23a, 0x7632),
+                                           __byte_perm(t01b, t23b, 0x5410), __byte_perm(t01b, t23b, 0x7632)};
 #pragma unroll
-            for (int ro = 0; ro < 4; ++ro) {
-                uint32_t o[12];
-#pragma unroll
-                for (int m = 0; m < 12; ++m) {
-                    if (INV) {  // row-major: row ro, bytes 4m .. 4m+3 of the 48
-                        const int x0 = 4 * m, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3;
-                        o[m] = gather4(R + ro * 12, (x0 % 3) * 4 + ((x0 / 3) >> 2), (x0 / 3) & 3, (x1 % 3) * 4 + ((x1 / 3) >> 2),
-                                       (x1 / 3) & 3, (x2 % 3) * 4 + ((x2 / 3) >> 2), (x2 / 3) & 3,
-                                       (x3 % 3) * 4 + ((x3 / 3) >> 2), (x3 / 3) & 3);
-                    } else {  // T4: block row ro, word m = byte column 4m + ro of rows 0..3
-                        const int x = 4 * m + ro, ri = (x % 3) * 4 + ((x / 3) >> 2), by = (x / 3) & 3;
-                        o[m] = gather4(R, ri, by, 12 + ri, by, 24 + ri, by, 36 + ri, by);
+                    for (int p = 0; p < 4; ++p) {
+                        const int y = 3 * p + ch;
+                        *reinterpret_cast<uint32_t *>(o + (y & 3) * rb + 4 * (y >> 2)) = T[p];
                     }
                 }
-                uint4 *po = reinterpret_cast<uint4 *>(stage + ro * rb + 48u * k);
-                po[0] = make_uint4(o[0], o[1], o[2], o[3]);
-                po[1] = make_uint4(o[4], o[5], o[6], o[7]);
-                po[2] = make_uint4(o[8], o[9], o[10], o[11]);
+            } else {
+                // row-major: byte y = 3 * pixel + channel of the quad's 12 bytes
+#pragma unroll
+                for (int r = 0; r < ROW_RB; ++r) {
+                    uint32_t *po = reinterpret_cast<uint32_t *>(o + r * rb);
+                    po[0] = __byte_perm(__byte_perm(R[r][0], R[r][1], 0x1040), R[r][2], 0x3410);
+                    po[1] = __byte_perm(__byte_perm(R[r][0], R[r][1], 0x6205), R[r][2], 0x3250);
+                    po[2] = __byte_perm(__byte_perm(R[r][0], R[r][1], 0x0730), R[r][2], 0x7216);
+                }
             }
         }
-        if (tid < 3 * ROW_RB) par[((it + 1u) & 1u) * 16u + tid] = pnext;
-        fence_async_smem();  // generic-proxy writes to the stage -> visible to the bulk store
-        __syncthreads();
-        if (tid == 0) {
-            bulk_s2g(dst + (size_t)blk * blk_bytes, stage, blk_bytes);
-            const uint32_t nb = blk + 2u * G;
-            if (nb < nblocks) {
-                const uint32_t s2 = s >= 1 ? s - 1 : ROW_NBUF - 1;  // (s + 2) % 3: the buffer of block it - 1
-                bulk_wait_read_1();                                 // its store has left shared memory
-                mbar_expect_tx(bar + s2, blk_bytes);
-                bulk_g2s(stage0 + s2 * blk_bytes, src + (size_t)nb * blk_bytes, blk_bytes, bar + s2);
-            }
-        }
-        s = s + 1 == ROW_NBUF ? 0 : s + 1;
+        fence_async_smem();     // generic-proxy writes to the stage -> visible to the bulk store
+        named_bar_sync(1, NC);  // block complete; planes free for the next block
+        if (tid == 0) mbar_arrive(done + s);
+        if (++s == NS) { s = 0; ph ^= 1u; }
     }
-    if (tid == 0) bulk_wait_all();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Column pass, encrypt direction: vertical circular shift of every byte column (Algorithm 5 / Eq. 3, one
+// d_v per pixel column and channel = per byte column of the interleaved matrix) fused with the XOR of
+// Algorithm 6:   dst(ro, x) = B(ro, x) xor I((ro - t_x) mod h, x),   I = the row pass output in T4 layout.
+// One CTA = one strip of X byte columns of one frame, all h rows (+ 8 repeated rows so that a window never
+// wraps) in shared memory, brought in by the TMA engine as 2-D tensor tiles (cp.async.bulk.tensor ->
+// UTMALDG): no thread touches the strip on its way in.  In T4 layout ONE 32-bit shared-memory load returns
+// four consecutive rows of a byte column, so 8 output rows of a column cost 3 loads + 2 funnel shifts.
+// A warp is split into NSUB = 256 / X sub-warps of X / 8 lanes; a lane owns 8 byte columns (two T4 word
+// columns x four byte lanes) and a sub-warp emits groups of 8 consecutive output rows with 64-bit
+// keystream loads and ciphertext stores.  Bank of a load = (strip row * X/4 + word column) mod 32 with strip
+// row = 4R + b: sub-warp s walks its columns in the order (word column a_l ^ (s & 1), byte lane a_b ^ (s >> 1)),
+// so the sub-warps of a warp always sit in disjoint banks whatever rows they read: no conflicts for
+// X = 128, 64, 32.  The permutation is undone by the selectors of the 4 x 4 byte transposes and by one
+// select per output word.
+// In place is safe: the whole strip is in shared memory before the first store.
+// ---------------------------------------------------------------------------------------------
+constexpr int CE_PAD = 8;   // repeated strip rows
+constexpr int CE_G = 8;     // output rows per group
+
+__device__ __forceinline__ void tma_load_2d(void *smem_dst, const CUtensorMap *tm, int32_t x, int32_t y, uint64_t *bar,
+                                            uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4}], [%2], %5;" ::
+            "r"(smem_u32(smem_dst)),
+        "l"(reinterpret_cast<uint64_t>(tm)), "r"(smem_u32(bar)), "r"(x), "r"(y), "l"(pol)
+        : "memory");
+}
+
+// p + off as one IMAD.WIDE.U32 (FMA pipe) instead of a two-instruction 64-bit add on the ALU pipe
+__device__ __forceinline__ uint64_t mad_wide_ptr(const void *p, uint32_t off) {
+    uint64_t r;
+    asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(r) : "r"(off), "l"(reinterpret_cast<uint64_t>(p)));
+    return r;
+}
+
+template <int X, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
+    col_enc_kernel(const __grid_constant__ CUtensorMap tm_main, const __grid_constant__ CUtensorMap tm_pad,
+                   const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
+                   uint32_t strips_per_frame, uint32_t nframes, uint32_t box_rows, uint32_t h_magic) {
+    extern __shared__ __align__(128) uint8_t S[];
+    constexpr uint32_t LPS = X / 8;       // lanes per strip row
+    constexpr uint32_t NSUB = 32 / LPS;   // sub-warps per warp
+    constexpr uint32_t NW = NT / 32;
+    constexpr uint32_t GSTEP = NW * NSUB;  // groups between two iterations of a sub-warp
+    const uint32_t h = g.h, rb = g.row_bytes;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(S + (size_t)(h + CE_PAD) * X);
+    uint16_t *ups = reinterpret_cast<uint16_t *>(S + (size_t)(h + CE_PAD) * X + 16);  // [X] source row offset per byte column
+    // the last frame first: its intermediate was written last and is the most likely to be in L2
+    const uint32_t fr = blockIdx.x / strips_per_frame;
+    const uint32_t f = nframes - 1u - fr;
+    const uint32_t x0 = (blockIdx.x - fr * strips_per_frame) * X;
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        const uint64_t pol = policy_evict_first();
+        mbar_expect_tx(bar, (h + CE_PAD) * X);
+        const int32_t y0 = (int32_t)(f * h);
+        for (uint32_t r0 = 0; r0 < h; r0 += box_rows) tma_load_2d(S + (size_t)r0 * X, &tm_main, (int32_t)x0, y0 + (int32_t)r0, bar, pol);
+        tma_load_2d(S + (size_t)h * X, &tm_pad, (int32_t)x0, y0, bar, pol);
+    }
+    // one thread per byte column of the strip: up = (h - d_v mod h) mod h, the row offset of the column's source
+    if (threadIdx.x >= NT - X) {
+        const uint32_t xs = threadIdx.x - (NT - X);
+        uint32_t x = x0 + xs;
+        if (x >= rb) x = 0;
+        const uint32_t jj = x / 3u, c = x - 3u * jj;
+        const uint32_t dv = D[(size_t)f * g.nD + c * (h + g.w) + h + jj];
+        const uint32_t t = dv - __umulhi(dv, h_magic) * h;  // d_v mod h  (h_magic = ceil(2^32 / h), d_v < 2^16)
+        ups[xs] = (uint16_t)(t ? h - t : 0u);
+    }
+
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t sub = lane / LPS, j = lane % LPS;
+    const uint32_t sl = sub & 1u, sb = sub >> 1;   // permutation of the word column / byte lane order
+    const uint32_t xt = x0 + 8u * j;               // first of this lane's 8 byte columns (frame coordinates)
+    const bool col_ok = xt < rb;                   // rb % 8 == 0 on this path: the 8 columns are inside or outside together
+    const uint32_t g0 = warp * NSUB + sub;         // first group of this sub-warp
+    const uint32_t nfull = h / CE_G;               // full groups; h % 8 == 4 leaves one half group
+    const bool active = col_ok && g0 * CE_G < h;
+    const size_t fbase = (size_t)f * g.frame_bytes + xt + (size_t)(g0 * CE_G) * rb;
+    const uint8_t *pB = Bk + fbase;                // row g0 * 8 of this lane's columns
+    uint8_t *pO = dst + fbase;
+    const uint32_t rb2 = 2u * rb, rb3 = 3u * rb, rb4 = 4u * rb, rb5 = 5u * rb, rb6 = 6u * rb, rb7 = 7u * rb;
+    const size_t gstep = (size_t)(GSTEP * CE_G) * rb;
+
+#define VK_ROWPTR(T, P, OFF) reinterpret_cast<T>(mad_wide_ptr(P, OFF))
+    // keystream of the first group: issued before the strip arrives
+    uint2 kb[CE_G];
+#pragma unroll
+    for (int i = 0; i < CE_G; ++i) kb[i] = make_uint2(0u, 0u);
+    if (active) {
+        const uint32_t offs[8] = {0u, rb, rb2, rb3, rb4, rb5, rb6, rb7};
+        if (g0 < nfull) {
+#pragma unroll
+            for (int i = 0; i < CE_G; ++i) kb[i] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[i]));
+        } else {
+#pragma unroll
+            for (int i = 0; i < CE_G / 2; ++i) kb[i] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[i]));
+        }
+    }
+    __syncthreads();  // mbarrier initialised, ups[] complete
+
+    // per step a = (a_l, a_b): state of byte column 4 * (2j + (a_l ^ sl)) + (a_b ^ sb) of the strip.
+    // q = byte offset of the aligned source block row in the strip (a multiple of 4X) | 8j | K_s | row alignment
+    // (low 2 bits); the T4 word of the column sits at (q & ~3) ^ K_a  with  K = byte lane * X + 4 * word column bit.
+    const uint32_t hX = h * X;
+    const uint32_t ADVX = ((GSTEP * CE_G) % h) * X;  // strip bytes between two iterations (h % 4 == 0 keeps alignment)
+    const uint32_t Ks = sb * X + 4u * sl;
+    uint32_t q[8];
+    {
+        // the lane's 8 offsets in natural order (two per word), then permuted into walking order a -> a ^ (4 sl + sb)
+        const uint4 u4 = *reinterpret_cast<const uint4 *>(ups + 8u * j);
+        uint32_t u[4] = {u4.x, u4.y, u4.z, u4.w};
+        const uint32_t sw = (sb & 1u) ? 0x1032u : 0x3210u;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) u[k] = __byte_perm(u[k], 0u, sw);
+        if (sb & 2u) { uint32_t t0 = u[0]; u[0] = u[1]; u[1] = t0; t0 = u[2]; u[2] = u[3]; u[3] = t0; }
+        if (sl) { uint32_t t0 = u[0]; u[0] = u[2]; u[2] = t0; t0 = u[1]; u[1] = u[3]; u[3] = t0; }
+        const uint32_t base = (8u * j) | Ks;
+        uint32_t ro0 = g0 * CE_G;
+        if (ro0 >= h) ro0 = 0;
+#pragma unroll
+        for (int a = 0; a < 8; ++a) {
+            const uint32_t up = (a & 1) ? (u[a >> 1] >> 16) : (u[a >> 1] & 0xFFFFu);
+            uint32_t s0 = ro0 + up;
+            if (s0 >= h) s0 -= h;
+            q[a] = (s0 & ~3u) * X + (base | (s0 & 3u));
+        }
+    }
+    // transpose selectors: in[0], in[1] hold byte lanes (sb&1, sb&1 ^ 1); in[2], in[3] the other pair
+    const uint32_t selA = (sb & 1u) ? 0x1504u : 0x5140u, selB = (sb & 1u) ? 0x3726u : 0x7362u;
+    const uint32_t selLo = (sb & 2u) ? 0x1054u : 0x5410u, selHi = (sb & 2u) ? 0x3276u : 0x7632u;
+    const uint32_t m3 = ~3u;
+
+    mbar_wait(bar, 0);  // strip (and its wrap rows) has landed
+    if (!active) return;
+
+    for (uint32_t gi = g0;; gi += GSTEP) {
+        uint32_t O[CE_G][2];
+#pragma unroll
+        for (int al_ = 0; al_ < 2; ++al_) {
+            uint32_t A[4][2];
+#pragma unroll
+            for (int ab = 0; ab < 4; ++ab) {
+                const int a = al_ * 4 + ab;
+                const uint32_t Ka = (uint32_t)ab * X + 4u * (uint32_t)al_;
+                const uint8_t *p = S + ((q[a] & m3) ^ Ka);
+                const uint32_t r0 = *reinterpret_cast<const uint32_t *>(p);
+                const uint32_t r1 = *reinterpret_cast<const uint32_t *>(p + 4 * X);
+                const uint32_t r2 = *reinterpret_cast<const uint32_t *>(p + 8 * X);
+                const uint32_t shamt = q[a] << 3;  // funnel shift uses the low 5 bits: 8 * alignment
+                A[ab][0] = __funnelshift_r(r0, r1, shamt);
+                A[ab][1] = __funnelshift_r(r1, r2, shamt);
+                q[a] += ADVX;
+                if (q[a] >= hX) q[a] -= hX;
+            }
+#pragma unroll
+            for (int hg = 0; hg < 2; ++hg) {
+                const uint32_t t01a = __byte_perm(A[0][hg], A[1][hg], selA), t01b = __byte_perm(A[0][hg], A[1][hg], selB);
+                const uint32_t t23a = __byte_perm(A[2][hg], A[3][hg], selA), t23b = __byte_perm(A[2][hg], A[3][hg], selB);
+                O[4 * hg + 0][al_] = __byte_perm(t01a, t23a, selLo);
+                O[4 * hg + 1][al_] = __byte_perm(t01a, t23a, selHi);
+                O[4 * hg + 2][al_] = __byte_perm(t01b, t23b, selLo);
+                O[4 * hg + 3][al_] = __byte_perm(t01b, t23b, selHi);
+            }
+        }
+        // undo the word column permutation, xor the keystream, store
+        const uint32_t offs[8] = {0u, rb, rb2, rb3, rb4, rb5, rb6, rb7};
+        if (gi < nfull) {
+#pragma unroll
+            for (int i = 0; i < CE_G; ++i) {
+                const uint32_t lo = sl ? O[i][1] : O[i][0], hi = sl ? O[i][0] : O[i][1];
+                __stcs(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[i].x, hi ^ kb[i].y));
+            }
+        } else {  // the half group at the bottom of a frame with h % 8 == 4: always the last one
+#pragma unroll
+            for (int i = 0; i < CE_G / 2; ++i) {
+                const uint32_t lo = sl ? O[i][1] : O[i][0], hi = sl ? O[i][0] : O[i][1];
+                __stcs(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[i].x, hi ^ kb[i].y));
+            }
+            break;
+        }
+        // keystream of the next group
+        const uint32_t gn = gi + GSTEP;
+        if (gn * CE_G >= h) break;
+        pB += gstep;
+        pO += gstep;
+        if (gn < nfull) {
+#pragma unroll
+            for (int i = 0; i < CE_G; ++i) kb[i] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[i]));
+        } else {
+#pragma unroll
+            for (int i = 0; i < CE_G / 2; ++i) kb[i] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[i]));
+        }
+    }
+#undef VK_ROWPTR
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -553,19 +838,24 @@ __global__ void __launch_bounds__(256)
 // ---------------------------------------------------------------------------------------------
 // host side: plan + launches
 // ---------------------------------------------------------------------------------------------
-static size_t row_smem_bytes(const Geom &g) {
-    const size_t C = g.w / 16;
-    return (size_t)ROW_HDR + (size_t)ROW_NBUF * ROW_RB * g.row_bytes + (size_t)ROW_RB * 3 * 20 * (C + 1);
+static size_t row_smem_bytes(const Geom &g, int ns) {
+    return (size_t)ROW_HDR + (size_t)ns * ROW_RB * g.row_bytes + (size_t)ROW_RB * 3 * (g.w + 32);
 }
 static size_t col_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + COL_PAD) * X; }
+static size_t cole_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + CE_PAD) * X + 16 + 2 * (size_t)X; }
 
 template <int X, int NT, int MINB>
 static cudaError_t col_set_attr(size_t smem) {
-    cudaError_t e = cudaFuncSetAttribute(col_pass_kernel<X, false, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(col_pass_kernel<X, true, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    return e;
+    return cudaFuncSetAttribute(col_pass_kernel<X, true, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
 }
+template <int X, int NT, int MINB>
+static cudaError_t cole_set_attr(size_t smem) {
+    return cudaFuncSetAttribute(col_enc_kernel<X, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 cudaError_t make_plan(const Geom &g, int device, Plan *out) {
     Plan p{};
@@ -576,41 +866,75 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
     if (e != cudaSuccess) return e;
     p.tiled = false;
     p.max_frames_per_launch = 1;
-    if (g.w % 16 == 0 && g.h % 4 == 0 && g.h >= 2 * COL_PAD) {
-        // column strip: the widest X that leaves room for 3 CTAs per SM (256 threads each); else the
+    const bool shape_ok = g.w % 16 == 0 && g.h % 4 == 0 && g.h >= 2 * COL_PAD && g.w >= 64 &&
+                          g.frame_bytes < ((size_t)1 << 31);
+    if (shape_ok) {
+        // column strips: the widest X that leaves room for 3 CTAs per SM (256 threads each); else the
         // widest that fits at all (one CTA of 512 threads per SM)
         const int cands[3] = {128, 64, 32};
         int X = 0, ctas = 0;
         for (int c = 0; c < 3 && !X; ++c)
-            if (3 * (col_smem_bytes(g, cands[c]) + 1024) <= (size_t)smem_sm) { X = cands[c]; ctas = 3; }
+            if (3 * (cole_smem_bytes(g, cands[c]) + 1024) <= (size_t)smem_sm) { X = cands[c]; ctas = 3; }
         for (int c = 0; c < 3 && !X; ++c)
-            if (col_smem_bytes(g, cands[c]) <= (size_t)smem_optin) { X = cands[c]; ctas = 1; }
-        p.smem_row = row_smem_bytes(g);
-        if (X && p.smem_row <= (size_t)smem_optin) {
+            if (cole_smem_bytes(g, cands[c]) <= (size_t)smem_optin) { X = cands[c]; ctas = 1; }
+        // row pass: compute threads = one per quad of 4 pixels, at most 15 warps (+ the copy warp) when
+        // several CTAs share an SM; the deepest ring of stages that still leaves 2 CTAs per SM, else what fits
+        const uint32_t Q = g.w / 4;
+        int nc = (int)(((Q + 31) / 32) * 32);
+        if (nc > 480) nc = 480;
+        int ns = 0;
+        for (int cand = 3; cand >= 2 && !ns; --cand)
+            if (2 * (row_smem_bytes(g, cand) + 1024) <= (size_t)smem_sm) ns = cand;
+        bool row_big = false;
+        if (!ns) {
+            for (int cand = 3; cand >= 1 && !ns; --cand)
+                if (row_smem_bytes(g, cand) <= (size_t)smem_optin) ns = cand;
+            row_big = true;
+            nc = (int)(((Q + 31) / 32) * 32);
+            if (nc > 992) nc = 992;
+        }
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (X && ns && cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess && fn) {
             p.tiled = true;
+            p.encode_tiled = fn;
             p.strip_bytes = X;
             p.col_ctas_per_sm = ctas;
             p.strips_per_frame = (int)((g.row_bytes + X - 1) / X);
             p.smem_col = col_smem_bytes(g, X);
-            p.row_threads = g.w / 16 <= 128 ? (int)(((g.w / 16 + 31) / 32) * 32) : 256;
+            p.smem_cole = cole_smem_bytes(g, X);
+            uint32_t br = 1;
+            for (uint32_t d = 1; d <= 256 && d <= g.h; ++d)
+                if (g.h % d == 0) br = d;
+            p.box_rows = br;
+            p.h_magic = (uint32_t)((((uint64_t)1 << 32) + g.h - 1) / g.h);
+            p.row_ns = ns;
+            p.row_nc = nc;
+            p.row_big = row_big;
+            p.smem_row = row_smem_bytes(g, ns);
             int rc = (int)((size_t)smem_sm / (p.smem_row + 1024));
-            if (rc > 4) rc = 4;
-            if (rc < 1) rc = 1;
+            const int by_threads = 2048 / (nc + 32);
+            if (rc > by_threads) rc = by_threads;
+            if (rc > 3) rc = 3;
+            if (rc < 1 || row_big) rc = 1;
             p.row_grid_max = rc * sms;
             const size_t l2_budget = (size_t)56 << 20;  // intermediate kept well inside the 126 MB L2
             p.max_frames_per_launch = l2_budget / g.frame_bytes ? l2_budget / g.frame_bytes : 1;
             if (ctas == 3) {
-                if (X == 128) e = col_set_attr<128, 256, 3>(p.smem_col);
-                else if (X == 64) e = col_set_attr<64, 256, 3>(p.smem_col);
-                else e = col_set_attr<32, 256, 3>(p.smem_col);
+                if (X == 128) { e = col_set_attr<128, 256, 3>(p.smem_col); if (!e) e = cole_set_attr<128, 256, 3>(p.smem_cole); }
+                else if (X == 64) { e = col_set_attr<64, 256, 3>(p.smem_col); if (!e) e = cole_set_attr<64, 256, 3>(p.smem_cole); }
+                else { e = col_set_attr<32, 256, 3>(p.smem_col); if (!e) e = cole_set_attr<32, 256, 3>(p.smem_cole); }
             } else {
-                if (X == 128) e = col_set_attr<128, 512, 1>(p.smem_col);
-                else if (X == 64) e = col_set_attr<64, 512, 1>(p.smem_col);
-                else e = col_set_attr<32, 512, 1>(p.smem_col);
+                if (X == 128) { e = col_set_attr<128, 512, 1>(p.smem_col); if (!e) e = cole_set_attr<128, 512, 1>(p.smem_cole); }
+                else if (X == 64) { e = col_set_attr<64, 512, 1>(p.smem_col); if (!e) e = cole_set_attr<64, 512, 1>(p.smem_cole); }
+                else { e = col_set_attr<32, 512, 1>(p.smem_col); if (!e) e = cole_set_attr<32, 512, 1>(p.smem_cole); }
             }
             if (e != cudaSuccess) return e;
-            e = cudaFuncSetAttribute(row_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
-            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
+            e = cudaFuncSetAttribute(row_pass_kernel<false, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
+            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
+            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<false, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
+            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
             if (e != cudaSuccess) return e;
         }
     }
@@ -623,15 +947,19 @@ static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, 
                               uint8_t *dst, cudaStream_t st) {
     const uint32_t nblocks = (uint32_t)(n * g.h / ROW_RB);
     const uint32_t grid = nblocks < (uint32_t)p.row_grid_max ? nblocks : (uint32_t)p.row_grid_max;
-    row_pass_kernel<INV><<<grid, p.row_threads, p.smem_row, st>>>(src, dst, D, g, nblocks);
+    const uint32_t nt = (uint32_t)p.row_nc + 32u;
+    if (p.row_big)
+        row_pass_kernel<INV, 1024, 1><<<grid, nt, p.smem_row, st>>>(src, dst, D, g, nblocks, (uint32_t)p.row_ns, (uint32_t)p.row_nc);
+    else
+        row_pass_kernel<INV, 512, 2><<<grid, nt, p.smem_row, st>>>(src, dst, D, g, nblocks, (uint32_t)p.row_ns, (uint32_t)p.row_nc);
     return cudaGetLastError();
 }
 
-template <bool INV>
-static cudaError_t launch_col(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
-                              size_t n, uint8_t *dst, cudaStream_t st) {
+// decrypt direction (row-major in and out)
+static cudaError_t launch_col_inv(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
+                                  size_t n, uint8_t *dst, cudaStream_t st) {
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
-#define VK_COL(X, NT, MINB) col_pass_kernel<X, INV, NT, MINB><<<grid, NT, p.smem_col, st>>>(src, B, dst, D, g, p.strips_per_frame)
+#define VK_COL(X, NT, MINB) col_pass_kernel<X, true, NT, MINB><<<grid, NT, p.smem_col, st>>>(src, B, dst, D, g, p.strips_per_frame)
     if (p.col_ctas_per_sm == 3) {
         if (p.strip_bytes == 128) VK_COL(128, 256, 3);
         else if (p.strip_bytes == 64) VK_COL(64, 256, 3);
@@ -645,6 +973,38 @@ static cudaError_t launch_col(const Geom &g, const Plan &p, const uint8_t *src, 
     return cudaGetLastError();
 }
 
+// encrypt direction: the T4 intermediate in `io` is replaced by the ciphertext
+static cudaError_t launch_col_enc(const Geom &g, const Plan &p, uint8_t *io, const uint16_t *D, const uint8_t *B, size_t n,
+                                  cudaStream_t st) {
+    alignas(64) CUtensorMap tm_main, tm_pad;
+    const cuuint64_t dims[2] = {g.row_bytes, (cuuint64_t)n * g.h};
+    const cuuint64_t strides[1] = {g.row_bytes};
+    const cuuint32_t es[2] = {1, 1};
+    const cuuint32_t box_main[2] = {(cuuint32_t)p.strip_bytes, p.box_rows}, box_pad[2] = {(cuuint32_t)p.strip_bytes, CE_PAD};
+    EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(p.encode_tiled);
+    CUresult r = enc(&tm_main, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, io, dims, strides, box_main, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r == CUDA_SUCCESS)
+        r = enc(&tm_pad, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, io, dims, strides, box_pad, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
+#define VK_COLE(X, NT, MINB)                                                                                              \
+    col_enc_kernel<X, NT, MINB><<<grid, NT, p.smem_cole, st>>>(tm_main, tm_pad, B, io, D, g, (uint32_t)p.strips_per_frame, \
+                                                               (uint32_t)n, p.box_rows, p.h_magic)
+    if (p.col_ctas_per_sm == 3) {
+        if (p.strip_bytes == 128) VK_COLE(128, 256, 3);
+        else if (p.strip_bytes == 64) VK_COLE(64, 256, 3);
+        else VK_COLE(32, 256, 3);
+    } else {
+        if (p.strip_bytes == 128) VK_COLE(128, 512, 1);
+        else if (p.strip_bytes == 64) VK_COLE(64, 512, 1);
+        else VK_COLE(32, 512, 1);
+    }
+#undef VK_COLE
+    return cudaGetLastError();
+}
+
 cudaError_t encrypt_tiled(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
                           size_t n, uint8_t *dst, cudaStream_t st, int *launches) {
     for (size_t f0 = 0; f0 < n; f0 += p.max_frames_per_launch) {
@@ -652,7 +1012,7 @@ cudaError_t encrypt_tiled(const Geom &g, const Plan &p, const uint8_t *src, cons
         const size_t off = f0 * g.frame_bytes;
         cudaError_t e = launch_row<false>(g, p, src + off, D + f0 * g.nD, m, dst + off, st);
         if (e != cudaSuccess) return e;
-        e = launch_col<false>(g, p, dst + off, D + f0 * g.nD, B + off, m, dst + off, st);
+        e = launch_col_enc(g, p, dst + off, D + f0 * g.nD, B + off, m, st);
         if (e != cudaSuccess) return e;
         *launches += 2;
     }
@@ -664,7 +1024,7 @@ cudaError_t decrypt_tiled(const Geom &g, const Plan &p, const uint8_t *src, cons
     for (size_t f0 = 0; f0 < n; f0 += p.max_frames_per_launch) {
         const size_t m = n - f0 < p.max_frames_per_launch ? n - f0 : p.max_frames_per_launch;
         const size_t off = f0 * g.frame_bytes;
-        cudaError_t e = launch_col<true>(g, p, src + off, D + f0 * g.nD, B + off, m, dst + off, st);
+        cudaError_t e = launch_col_inv(g, p, src + off, D + f0 * g.nD, B + off, m, dst + off, st);
         if (e != cudaSuccess) return e;
         e = launch_row<true>(g, p, dst + off, D + f0 * g.nD, m, dst + off, st);
         if (e != cudaSuccess) return e;
