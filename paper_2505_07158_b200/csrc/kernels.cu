@@ -211,6 +211,12 @@ __device__ __forceinline__ uint2 row_param(const uint16_t *__restrict__ D, const
     return make_uint2((dw >> 2) << 4, ((plane_off + 4u * (dw & 3u)) << 8) | (sh & 31u));
 }
 
+// Programmatic dependent launch (PDL): a kernel launched with the programmatic-stream-serialization attribute may start
+// while its predecessor in the stream is still draining; pdl_wait() blocks until the predecessor has completed and its
+// writes are visible, pdl_trigger() lets the successor's CTAs be scheduled as soon as resources free up.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -247,24 +253,31 @@ template <bool INV, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src, uint8_t *dst, const uint16_t *__restrict__ D,
                                                            Geom g, uint32_t nblocks, uint32_t NS, uint32_t NC) {
     extern __shared__ __align__(128) uint8_t smem[];
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem);                // [ROW_MAXNS]
-    uint64_t *done = reinterpret_cast<uint64_t *>(smem + 64);           // [ROW_MAXNS]
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);                // [ROW_MAXNS] input stage loaded
+    uint64_t *empty = reinterpret_cast<uint64_t *>(smem + 32);          // [ROW_MAXNS] input stage consumed by phase 1
+    uint64_t *ofull = reinterpret_cast<uint64_t *>(smem + 64);          // output buffer written by phase 2
+    uint64_t *ofree = reinterpret_cast<uint64_t *>(smem + 72);          // output buffer read by the bulk store
     uint32_t *par1 = reinterpret_cast<uint32_t *>(smem + 128);          // [ROW_MAXNS][4 rows][4]  (64 B per stage)
     uint32_t *par2 = reinterpret_cast<uint32_t *>(smem + 128 + 64 * ROW_MAXNS);  // same shape
     const uint32_t w = g.w, rb = g.row_bytes, C = w >> 4, Q = w >> 2;   // items / quads per row
     const uint32_t blk_bytes = ROW_RB * rb;
     const uint32_t PS = w + 32u;                                        // plane stride (bytes): w/4 words + 2 pad chunks
-    uint8_t *stage0 = smem + ROW_HDR;
-    uint8_t *planes = stage0 + NS * blk_bytes;
+    uint8_t *stage0 = smem + ROW_HDR;                                   // NS input stages
+    uint8_t *obuf = stage0 + NS * blk_bytes;                            // one output buffer
+    uint8_t *planes = obuf + blk_bytes;
     const uint32_t G = gridDim.x, tid = threadIdx.x;
     const uint32_t blk0 = blockIdx.x;
     if (blk0 >= nblocks) return;
     const uint32_t niter = (nblocks - blk0 + G - 1) / G;
 
     if (tid == 0) {
-        for (uint32_t s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(done + s, 1); }
+        for (uint32_t s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        mbar_init(ofull, 1);
+        mbar_init(ofree, 1);
     }
     __syncthreads();
+    pdl_wait();     // everything below reads or writes global memory the previous kernel of the stream may have written
+    pdl_trigger();  // only now: the column pass reads its keystream before its own wait, so it must not start before this point
 
     if (tid >= NC) {
         // ================= copy warp =================
@@ -290,22 +303,25 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
         for (uint32_t it = 0; it < niter; ++it) {
             const uint32_t blk = blk0 + it * G;
             const bool refill = it + NS < niter;
-            uint2 pnext = make_uint2(0u, 0u);
-            if (refill && lane < 3 * ROW_RB) pnext = row_param(D, g, (blk + NS * G) * ROW_RB + pr, pch, INV, poff);
-            if (lane == 0) {
-                mbar_wait(done + s, ph);  // the compute threads have written block `it` back into the stage
-                bulk_s2g(dst + (size_t)blk * blk_bytes, stage0 + s * blk_bytes, blk_bytes);
-            }
-            __syncwarp();
             if (refill) {
+                uint2 pnext = make_uint2(0u, 0u);
+                if (lane < 3 * ROW_RB) pnext = row_param(D, g, (blk + NS * G) * ROW_RB + pr, pch, INV, poff);
+                if (lane == 0) mbar_wait(empty + s, ph);  // phase 1 and phase 2 of block `it` no longer need stage s / its parameters
+                __syncwarp();
                 if (lane < 3 * ROW_RB) { par1[s * 16u + pslot] = pnext.x; par2[s * 16u + pslot] = pnext.y; }
                 __syncwarp();
                 if (lane == 0) {
-                    bulk_wait_read_0();  // the store has left shared memory
                     mbar_expect_tx(full + s, blk_bytes);
                     bulk_g2s_hint(stage0 + s * blk_bytes, src + (size_t)(blk + NS * G) * blk_bytes, blk_bytes, full + s, pol_in);
                 }
             }
+            if (lane == 0) {
+                mbar_wait(ofull, it & 1u);  // the compute threads have written block `it` into the output buffer
+                bulk_s2g(dst + (size_t)blk * blk_bytes, obuf, blk_bytes);
+                bulk_wait_read_0();         // the store has left shared memory
+                mbar_arrive(ofree);
+            }
+            __syncwarp();
             if (++s == NS) { s = 0; ph ^= 1u; }
         }
         if (lane == 0) bulk_wait_all();
@@ -317,7 +333,7 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
     const uint32_t r1 = (tid >= C) + (tid >= 2u * C) + (tid >= 3u * C), k1 = tid - r1 * C;
     uint32_t s = 0, ph = 0;
     for (uint32_t it = 0; it < niter; ++it) {
-        uint8_t *stage = stage0 + s * blk_bytes;
+        const uint8_t *stage = stage0 + s * blk_bytes;
         const uint32_t *p1 = par1 + s * 16u, *p2 = par2 + s * 16u;
         mbar_wait(full + s, ph);
 
@@ -354,7 +370,13 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
             VK_PUT(v2, dq.z, 2u)
 #undef VK_PUT
         }
-        named_bar_sync(1, NC);  // planes complete; the raw block in `stage` may now be overwritten
+        // the 12 phase-2 parameters of this block: read them before the stage (and its parameter slot) is released
+        uint4 pv[ROW_RB];
+#pragma unroll
+        for (int r = 0; r < ROW_RB; ++r) pv[r] = *reinterpret_cast<const uint4 *>(p2 + 4 * r);
+        named_bar_sync(1, NC);  // planes complete, raw block consumed
+        if (tid == 0) mbar_arrive(empty + s);
+        if (it > 0) mbar_wait(ofree, (it - 1u) & 1u);  // the previous block's store has left the output buffer
 
         // ---- phase 2: rotate; item = quad q (4 pixels) of all 4 rows and 3 channels
         for (uint32_t q = tid; q < Q; q += NC) {
@@ -362,15 +384,14 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
             uint32_t R[ROW_RB][3];
 #pragma unroll
             for (int r = 0; r < ROW_RB; ++r) {
-                const uint4 pv = *reinterpret_cast<const uint4 *>(p2 + 4 * r);
-                const uint32_t pvv[3] = {pv.x, pv.y, pv.z};
+                const uint32_t pvv[3] = {pv[r].x, pv[r].y, pv[r].z};
 #pragma unroll
                 for (int ch = 0; ch < 3; ++ch) {
                     const uint32_t *P = reinterpret_cast<const uint32_t *>(qa + (pvv[ch] >> 8));
                     R[r][ch] = __funnelshift_r(P[0], P[1], pvv[ch]);  // shift amount = low 5 bits
                 }
             }
-            uint8_t *o = stage + 12u * q;
+            uint8_t *o = obuf + 12u * q;
             if (!INV) {
                 // T4: pixel p of the quad, channel ch = byte column x = 12q + 3p + ch -> block row x & 3, word x >> 2
 #pragma unroll
@@ -396,9 +417,9 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
                 }
             }
         }
-        fence_async_smem();     // generic-proxy writes to the stage -> visible to the bulk store
+        fence_async_smem();     // generic-proxy writes to the output buffer -> visible to the bulk store
         named_bar_sync(1, NC);  // block complete; planes free for the next block
-        if (tid == 0) mbar_arrive(done + s);
+        if (tid == 0) mbar_arrive(ofull);
         if (++s == NS) { s = 0; ph ^= 1u; }
     }
 }
@@ -457,8 +478,10 @@ __global__ void __launch_bounds__(NT, MINB)
     const uint32_t f = nframes - 1u - fr;
     const uint32_t x0 = (blockIdx.x - fr * strips_per_frame) * X;
 
+    pdl_trigger();
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
+        pdl_wait();  // the strip is the row pass's output
         const uint64_t pol = policy_evict_first();
         mbar_expect_tx(bar, (h + CE_PAD) * X);
         const int32_t y0 = (int32_t)(f * h);
@@ -539,7 +562,7 @@ __global__ void __launch_bounds__(NT, MINB)
     const uint32_t selLo = (sb & 2u) ? 0x1054u : 0x5410u, selHi = (sb & 2u) ? 0x3276u : 0x7632u;
     const uint32_t m3 = ~3u;
 
-    mbar_wait(bar, 0);  // strip (and its wrap rows) has landed
+    mbar_wait(bar, 0);  // strip (and its wrap rows) has landed: the previous kernel has completed (thread 0 waited for it)
     if (!active) return;
 
     for (uint32_t gi = g0;; gi += GSTEP) {
@@ -839,7 +862,7 @@ __global__ void __launch_bounds__(256)
 // host side: plan + launches
 // ---------------------------------------------------------------------------------------------
 static size_t row_smem_bytes(const Geom &g, int ns) {
-    return (size_t)ROW_HDR + (size_t)ns * ROW_RB * g.row_bytes + (size_t)ROW_RB * 3 * (g.w + 32);
+    return (size_t)ROW_HDR + (size_t)(ns + 1) * ROW_RB * g.row_bytes + (size_t)ROW_RB * 3 * (g.w + 32);
 }
 static size_t col_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + COL_PAD) * X; }
 static size_t cole_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + CE_PAD) * X + 16 + 2 * (size_t)X; }
@@ -942,6 +965,23 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
     return cudaSuccess;
 }
 
+// Launch with programmatic stream serialization (PDL): the kernel's prologue may overlap the tail of the previous kernel
+// in the stream; every kernel launched this way calls pdl_wait() before it touches global memory that kernel may have written.
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kernel)(KArgs...), uint32_t grid, uint32_t block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 template <bool INV>
 static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, size_t n,
                               uint8_t *dst, cudaStream_t st) {
@@ -949,10 +989,10 @@ static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, 
     const uint32_t grid = nblocks < (uint32_t)p.row_grid_max ? nblocks : (uint32_t)p.row_grid_max;
     const uint32_t nt = (uint32_t)p.row_nc + 32u;
     if (p.row_big)
-        row_pass_kernel<INV, 1024, 1><<<grid, nt, p.smem_row, st>>>(src, dst, D, g, nblocks, (uint32_t)p.row_ns, (uint32_t)p.row_nc);
-    else
-        row_pass_kernel<INV, 512, 2><<<grid, nt, p.smem_row, st>>>(src, dst, D, g, nblocks, (uint32_t)p.row_ns, (uint32_t)p.row_nc);
-    return cudaGetLastError();
+        return launch_pdl(row_pass_kernel<INV, 1024, 1>, grid, nt, p.smem_row, st, src, dst, D, g, nblocks, (uint32_t)p.row_ns,
+                          (uint32_t)p.row_nc);
+    return launch_pdl(row_pass_kernel<INV, 512, 2>, grid, nt, p.smem_row, st, src, dst, D, g, nblocks, (uint32_t)p.row_ns,
+                      (uint32_t)p.row_nc);
 }
 
 // decrypt direction (row-major in and out)
@@ -989,9 +1029,9 @@ static cudaError_t launch_col_enc(const Geom &g, const Plan &p, uint8_t *io, con
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
-#define VK_COLE(X, NT, MINB)                                                                                              \
-    col_enc_kernel<X, NT, MINB><<<grid, NT, p.smem_cole, st>>>(tm_main, tm_pad, B, io, D, g, (uint32_t)p.strips_per_frame, \
-                                                               (uint32_t)n, p.box_rows, p.h_magic)
+#define VK_COLE(X, NT, MINB)                                                                                        \
+    return launch_pdl(col_enc_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_main, tm_pad, B, (uint8_t *)io, D, g, \
+                      (uint32_t)p.strips_per_frame, (uint32_t)n, p.box_rows, p.h_magic)
     if (p.col_ctas_per_sm == 3) {
         if (p.strip_bytes == 128) VK_COLE(128, 256, 3);
         else if (p.strip_bytes == 64) VK_COLE(64, 256, 3);
