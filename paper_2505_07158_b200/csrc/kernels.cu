@@ -13,26 +13,28 @@
 // followed by a per-byte-column circular shift in the interleaved H x 3W byte
 // matrix, followed by a byte XOR.  Two tiled passes do exactly that:
 //
-//   row pass    : work unit = a block of 4 rows; persistent CTAs run a three-buffer ring.  The rows
-//                 arrive in shared memory with one bulk async copy (TMA, cp.async.bulk), two blocks
-//                 ahead of the one being computed, are de-interleaved into three channel planes so
-//                 that the bit rotation becomes a 32-bit funnel shift of two neighbouring plane
-//                 words, and leave with one bulk async store.  When encrypting, the block is
-//                 written in the "T4" layout: the word at (row 4R + (x & 3), word column x >> 2)
-//                 holds byte column x of rows 4R .. 4R+3 -- a permutation inside the block, so the
-//                 intermediate still lives in the output buffer.
-//   column pass : a CTA owns a strip of X byte columns x all h rows in shared memory, in the T4
-//                 layout, so that ONE 32-bit shared-memory load returns four consecutive rows of a
-//                 byte column: 8 output rows of a column cost 3 conflict-free loads instead of 8
-//                 byte loads.  The words are byte-aligned and transposed back to row-major in
-//                 registers (PRMT), XORed with the keystream and streamed out.
+//   row pass    : work unit = a block of 4 rows.  Warp-specialised persistent CTAs: a copy warp brings
+//                 blocks in with bulk async copies (TMA, cp.async.bulk) into a ring of stages and sends
+//                 finished blocks out with bulk async stores; the compute warps de-interleave a block
+//                 into three channel planes (already rotated by the whole-chunk part of the distance),
+//                 so that the bit rotation becomes ONE 32-bit funnel shift of two neighbouring plane
+//                 words per output word.  When encrypting, the block is written in the "T4" layout: the
+//                 word at (row 4R + (x & 3), word column x >> 2) holds byte column x of rows 4R .. 4R+3
+//                 -- a permutation inside the block, so the intermediate still lives in the output buffer.
+//   column pass : a CTA owns a strip of 64 byte columns x all h rows in shared memory, in the T4 layout
+//                 (encrypt: brought in by TMA tensor tiles; decrypt: transposed in registers on the way
+//                 in), so that ONE 32-bit shared-memory load returns four consecutive rows of a byte
+//                 column: 8 output rows of a column cost 3 conflict-free loads + 2 funnel shifts.  The
+//                 words are transposed back to row-major in registers (PRMT), XORed with the keystream
+//                 (64-bit streaming loads) and streamed out (64-bit stores).
 //
 // The intermediate between the passes lives in the output buffer (every CTA of either pass reads all
 // of its rows / its whole strip before it writes them), and launches are sized so that it stays
 // resident in the 126 MB L2: DRAM traffic stays at the algorithmic read F_o + read B + write F_e.
+// The kernels of one call are chained with programmatic dependent launch (griddepcontrol).
 //
 // A one-thread-per-output-byte gather kernel covers every shape the tiled passes do not
-// (w % 16 != 0, h % 4 != 0, h < 16, or a strip / row block too large for shared memory).
+// (w % 16 != 0, w < 64, h % 4 != 0, h < 16, or a strip / row block too large for shared memory).
 #include <cuda.h>
 
 #include "kernels.cuh"
@@ -627,186 +629,194 @@ __global__ void __launch_bounds__(NT, MINB)
 }
 
 // ---------------------------------------------------------------------------------------------
-// Column pass: vertical circular shift of every byte column (Algorithm 5 / Eq. 3, one d_v per pixel
-// column and channel = per byte column of the interleaved matrix) fused with the XOR of Algorithm 6.
-//   INV = false:  dst(ro, x) = B(ro, x) xor I((ro - t_x) mod h, x)      src = I in T4 layout
-//   INV = true :  dst(i, x)  = (src xor B)((i + t_x) mod h, x)          src = F_e row-major; dst row-major
-// One CTA = one strip of X byte columns of one frame: h + 8 strip rows of X bytes in shared memory in T4
-// layout (strip row 4R + b, word l = rows 4R..4R+3 of byte column 4l + b; the last 8 strip rows repeat the
-// first 8 so that a window never wraps).  A warp is split into NSUB = 128 / X sub-warps of X / 4 lanes;
-// lane l of a sub-warp owns byte columns 4l .. 4l+3 of the strip and the sub-warp emits groups of 8
-// consecutive output rows: per byte column 3 word loads (12 source rows), a byte alignment (PRMT) and a
-// 4 x 4 byte transpose back to row-major words.  Bank of a load = (strip row * X/4 + l) mod 32 with strip
-// row = 4R + b, i.e. (b * X/4 + l) mod 32: sub-warp s walks the byte columns in the order b = a xor s, so
-// the sub-warps of a warp always sit in disjoint bank groups.  No conflicts for X = 128, 64, 32.
-// The keystream words of the next group are fetched while the current one is gathered.
-// In place is safe: phase A reads the whole strip before the barrier, phase B writes only that strip.
+// Column pass, decrypt direction: undo the XOR of Algorithm 6, then the vertical shift of
+// Algorithm 5:   dst(i, x) = (src xor B)((i + t_x) mod h, x),   src = F_e row-major, dst row-major (the
+// inverse row pass follows).  Same strip, same T4 layout in shared memory and the same conflict-free
+// gather as the encrypt direction; here the strip is filled by the threads themselves: 64-bit loads of
+// four rows of ciphertext and keystream, XOR, one 4 x 4 byte transpose per word column, 64-bit stores
+// (sub-warps take the byte lanes in the order b ^ (s & 1), so that two sub-warps together cover all banks).
+// In place is safe: the whole strip is in shared memory (barrier) before the first store.
 // ---------------------------------------------------------------------------------------------
-constexpr int COL_G = 8;    // output rows per group
-constexpr int COL_PAD = 8;  // repeated strip rows
-
-template <int X, bool INV, int NT, int MINB>
+template <int X, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
-    col_pass_kernel(const uint8_t *src, const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D,
-                    Geom g, int strips_per_frame) {
+    col_dec_kernel(const uint8_t *src, const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
+                   uint32_t strips_per_frame, uint32_t h_magic) {
     extern __shared__ __align__(128) uint8_t S[];
-    constexpr int LPR = X / 4;      // lanes per strip row
-    constexpr int NSUB = 32 / LPR;  // sub-warps per warp
-    constexpr int NW = NT / 32;
-    const uint32_t f = blockIdx.x / (uint32_t)strips_per_frame;
-    const uint32_t x0 = (blockIdx.x - f * (uint32_t)strips_per_frame) * X;
+    constexpr uint32_t LPS = X / 8;       // lanes per strip row
+    constexpr uint32_t NSUB = 32 / LPS;   // sub-warps per warp
+    constexpr uint32_t NW = NT / 32;
+    constexpr uint32_t GSTEP = NW * NSUB;  // row groups / row blocks between two iterations of a sub-warp
     const uint32_t h = g.h, rb = g.row_bytes;
-    const size_t fbase = (size_t)f * g.frame_bytes + x0;
-    const uint8_t *fsrc = src + fbase;
+    uint16_t *ups = reinterpret_cast<uint16_t *>(S + (size_t)(h + CE_PAD) * X + 16);  // [X] source row offset per byte column
+    const uint32_t f = blockIdx.x / strips_per_frame;
+    const uint32_t x0 = (blockIdx.x - f * strips_per_frame) * X;
+
+    pdl_wait();  // the ciphertext may be the previous kernel's output
+    pdl_trigger();
+    // one thread per byte column of the strip: t = d_v mod h, the row offset of the column's source
+    if (threadIdx.x >= NT - X) {
+        const uint32_t xs = threadIdx.x - (NT - X);
+        uint32_t x = x0 + xs;
+        if (x >= rb) x = 0;
+        const uint32_t jj = x / 3u, c = x - 3u * jj;
+        const uint32_t dv = D[(size_t)f * g.nD + c * (h + g.w) + h + jj];
+        ups[xs] = (uint16_t)(dv - __umulhi(dv, h_magic) * h);  // d_v mod h  (h_magic = ceil(2^32 / h), d_v < 2^16)
+    }
 
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t sub = lane / LPR, l = lane % LPR;
-    const uint32_t xw = x0 + 4u * l;  // first of this lane's 4 byte columns (frame coordinates)
-    const bool col_ok = xw < rb;      // rb % 4 == 0 on this path: a word is inside or outside as a whole
-    constexpr uint32_t GSTEP = NW * NSUB;  // groups between two iterations of a sub-warp
-    const uint32_t g0 = warp * NSUB + sub; // first group of this sub-warp
-    const uint32_t ngroups = (h + COL_G - 1) / COL_G;
-    // this lane's word in row r of the frame sits at word offset r * rw of these (32-bit indexing)
-    const uint32_t rw = rb >> 2;
-    const uint32_t *Bw = reinterpret_cast<const uint32_t *>(Bk + fbase) + l;
-    uint32_t *Ow = reinterpret_cast<uint32_t *>(dst + fbase) + l;
+    const uint32_t sub = lane / LPS, j = lane % LPS;
+    const uint32_t sl = sub & 1u, sb = sub >> 1;   // permutation of the word column / byte lane order (gather)
+    const uint32_t xt = x0 + 8u * j;               // first of this lane's 8 byte columns (frame coordinates)
+    const bool col_ok = xt < rb;
+    const uint32_t g0 = warp * NSUB + sub;
+    const size_t fcol = (size_t)f * g.frame_bytes + xt;
+    const uint32_t rb2 = 2u * rb, rb3 = 3u * rb, rb4 = 4u * rb, rb5 = 5u * rb, rb6 = 6u * rb, rb7 = 7u * rb;
+#define VK_ROWPTR(T, P, OFF) reinterpret_cast<T>(mad_wide_ptr(P, OFF))
 
-    // keystream words of the first group: issued before the strip arrives
-    uint32_t kb[COL_G];
+    // ---- phase A: (src xor B) -> T4 strip.  Item = (block of 4 rows R, this lane's 8 byte columns)
+    if (col_ok) {
+        const uint32_t s1 = sub & 1u;
+        const uint32_t selF = s1 ? 0x7632u : 0x5410u, selS = s1 ? 0x5410u : 0x7632u;  // first / second byte lane of a pair
+        const uint32_t nblk = h >> 2;
+        const uint8_t *pS = src + fcol + (size_t)(4u * g0) * rb;
+        const uint8_t *pB = Bk + fcol + (size_t)(4u * g0) * rb;
+        const size_t bstep = (size_t)(4u * GSTEP) * rb;
+        // software pipeline: the loads of the next block are in flight while this one is transposed and stored
+        const uint32_t offs[4] = {0u, rb, rb2, rb3};
+        uint2 vn[4], kn[4];
 #pragma unroll
-    for (int i = 0; i < COL_G; ++i) kb[i] = 0;
-    if (!INV && col_ok && g0 < ngroups) {
-        const uint32_t ro = g0 * COL_G;
+        for (int r = 0; r < 4; ++r) { vn[r] = make_uint2(0u, 0u); kn[r] = make_uint2(0u, 0u); }
+        if (g0 < nblk) {
 #pragma unroll
-        for (int i = 0; i < COL_G; ++i)
-            if (ro + i < h) kb[i] = __ldcs(Bw + (ro + i) * rw);
-    }
-
-    // ---- phase A: strip -> shared memory
-    if (!INV) {
-        constexpr int VPR = X / 16;  // 16-byte vectors per strip row
-        const uint32_t nvec = (h + COL_PAD) * VPR;
-        for (uint32_t v = threadIdx.x; v < nvec; v += NT) {
-            const uint32_t row = v / VPR, q = v % VPR;
-            const uint32_t srow = row < h ? row : row - h;
-            if (x0 + 16u * q < rb) cp_async16(S + (size_t)v * 16u, fsrc + (size_t)srow * rb + 16u * q);
-        }
-        cp_async_wait_all();
-    } else {
-        // row-major F_e xor B -> T4: one item = (block of 4 rows, word column)
-        const uint32_t nblk = (h + COL_PAD) >> 2, hb = h >> 2;
-        const uint32_t *Sw = reinterpret_cast<const uint32_t *>(fsrc);
-        const uint32_t *Bw0 = reinterpret_cast<const uint32_t *>(Bk + fbase);
-        for (uint32_t it = threadIdx.x; it < nblk * LPR; it += NT) {
-            const uint32_t R4 = it / LPR, ll = it % LPR;
-            const uint32_t sR = R4 < hb ? R4 : R4 - hb;
-            uint32_t v[4] = {0, 0, 0, 0}, o[4];
-            if (x0 + 4u * ll < rb) {
-                uint32_t kk[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const uint32_t off = (4u * sR + j) * rw + ll;
-                    v[j] = __ldcs(Sw + off);
-                    kk[j] = __ldcs(Bw0 + off);
-                }
-#pragma unroll
-                for (int j = 0; j < 4; ++j) v[j] ^= kk[j];
+            for (int r = 0; r < 4; ++r) {
+                vn[r] = __ldcs(VK_ROWPTR(const uint2 *, pS, offs[r]));
+                kn[r] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[r]));
             }
-            transpose4x4(v, o);
+        }
+        for (uint32_t R4 = g0; R4 < nblk; R4 += GSTEP) {
+            uint2 v[4], k[4];
 #pragma unroll
-            for (int b = 0; b < 4; ++b) *reinterpret_cast<uint32_t *>(S + ((size_t)(4u * R4 + b) * LPR + ll) * 4u) = o[b];
+            for (int r = 0; r < 4; ++r) { v[r] = vn[r]; k[r] = kn[r]; }
+            pS += bstep;
+            pB += bstep;
+            if (R4 + GSTEP < nblk) {
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    vn[r] = __ldcs(VK_ROWPTR(const uint2 *, pS, offs[r]));
+                    kn[r] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[r]));
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < 4; ++r) { v[r].x ^= k[r].x; v[r].y ^= k[r].y; }
+            // two 4 x 4 byte transposes: word column 2j (x) and 2j + 1 (y); outputs in the order b = t ^ s1
+            uint32_t lo[4], hi[4];
+            {
+                const uint32_t a = __byte_perm(v[0].x, v[1].x, 0x5140), b = __byte_perm(v[0].x, v[1].x, 0x7362);
+                const uint32_t c = __byte_perm(v[2].x, v[3].x, 0x5140), d = __byte_perm(v[2].x, v[3].x, 0x7362);
+                lo[0] = __byte_perm(a, c, selF); lo[1] = __byte_perm(a, c, selS);
+                lo[2] = __byte_perm(b, d, selF); lo[3] = __byte_perm(b, d, selS);
+            }
+            {
+                const uint32_t a = __byte_perm(v[0].y, v[1].y, 0x5140), b = __byte_perm(v[0].y, v[1].y, 0x7362);
+                const uint32_t c = __byte_perm(v[2].y, v[3].y, 0x5140), d = __byte_perm(v[2].y, v[3].y, 0x7362);
+                hi[0] = __byte_perm(a, c, selF); hi[1] = __byte_perm(a, c, selS);
+                hi[2] = __byte_perm(b, d, selF); hi[3] = __byte_perm(b, d, selS);
+            }
+            // step t holds byte lane b = t ^ s1: strip row 4 R4 + b, bytes 8j .. 8j+7
+            uint8_t *ps = S + ((size_t)(4u * R4) * X + 8u * j) + (s1 ? X : 0u);
+            const int32_t d1 = s1 ? -(int32_t)X : (int32_t)X;
+            *reinterpret_cast<uint2 *>(ps) = make_uint2(lo[0], hi[0]);
+            *reinterpret_cast<uint2 *>(ps + d1) = make_uint2(lo[1], hi[1]);
+            *reinterpret_cast<uint2 *>(ps + 2 * X) = make_uint2(lo[2], hi[2]);
+            *reinterpret_cast<uint2 *>(ps + 2 * X + d1) = make_uint2(lo[3], hi[3]);
+            if (R4 < CE_PAD / 4) {  // wrap rows: strip rows h .. h+7 repeat rows 0 .. 7
+                uint8_t *pw = ps + (size_t)h * X;
+                *reinterpret_cast<uint2 *>(pw) = make_uint2(lo[0], hi[0]);
+                *reinterpret_cast<uint2 *>(pw + d1) = make_uint2(lo[1], hi[1]);
+                *reinterpret_cast<uint2 *>(pw + 2 * X) = make_uint2(lo[2], hi[2]);
+                *reinterpret_cast<uint2 *>(pw + 2 * X + d1) = make_uint2(lo[3], hi[3]);
+            }
         }
     }
+    __syncthreads();  // strip and ups[] complete
 
-    // per byte column: source pointer, wrap limit, alignment selector
+    const uint32_t nfull = h / CE_G;
+    const bool active = col_ok && g0 * CE_G < h;
+    if (!active) return;
+    uint8_t *pO = dst + fcol + (size_t)(g0 * CE_G) * rb;
+    const size_t gstep = (size_t)(GSTEP * CE_G) * rb;
+
     const uint32_t hX = h * X;
-    constexpr uint32_t ADV = GSTEP * COL_G * X;  // bytes of strip between two iterations
-    uint32_t p[4], lim[4], sel[4];
+    const uint32_t ADVX = ((GSTEP * CE_G) % h) * X;
+    const uint32_t Ks = sb * X + 4u * sl;
+    uint32_t q[8];
     {
-        const uint16_t *Df = D + (size_t)f * g.nD;
+        const uint4 u4 = *reinterpret_cast<const uint4 *>(ups + 8u * j);
+        uint32_t u[4] = {u4.x, u4.y, u4.z, u4.w};
+        const uint32_t sw = (sb & 1u) ? 0x1032u : 0x3210u;
 #pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            const uint32_t b = (uint32_t)a ^ (sub & 3u);  // byte column walked at step a (NSUB <= 4)
-            uint32_t x = xw + b;
-            if (!col_ok) x = b;
-            const uint32_t j = x / 3u, c = x - 3u * j;
-            const uint32_t t = (uint32_t)Df[c * (h + g.w) + h + j] % h;
-            const uint32_t up = INV ? t : (t ? h - t : 0u);  // source row = (row + up) mod h
-            uint32_t s0 = (g0 * COL_G) % h + up;
+        for (int k = 0; k < 4; ++k) u[k] = __byte_perm(u[k], 0u, sw);
+        if (sb & 2u) { uint32_t t0 = u[0]; u[0] = u[1]; u[1] = t0; t0 = u[2]; u[2] = u[3]; u[3] = t0; }
+        if (sl) { uint32_t t0 = u[0]; u[0] = u[2]; u[2] = t0; t0 = u[1]; u[1] = u[3]; u[3] = t0; }
+        const uint32_t base = (8u * j) | Ks;
+        const uint32_t ro0 = g0 * CE_G;
+#pragma unroll
+        for (int a = 0; a < 8; ++a) {
+            const uint32_t up = (a & 1) ? (u[a >> 1] >> 16) : (u[a >> 1] & 0xFFFFu);
+            uint32_t s0 = ro0 + up;
             if (s0 >= h) s0 -= h;
-            const uint32_t al = s0 & 3u;
-            sel[a] = 0x3210u + 0x1111u * al;
-            const uint32_t cst = b * X + 4u * l;
-            p[a] = (s0 - al) * X + cst;
-            lim[a] = hX + cst;
+            q[a] = (s0 & ~3u) * X + (base | (s0 & 3u));
         }
     }
-    // transpose selectors: A[0], A[1] hold byte columns (s, s^1), A[2], A[3] hold (s^2, s^3)
-    const uint32_t selA = (sub & 1u) ? 0x1504u : 0x5140u, selB = (sub & 1u) ? 0x3726u : 0x7362u;
-    const uint32_t selLo = (sub & 2u) ? 0x1054u : 0x5410u, selHi = (sub & 2u) ? 0x3276u : 0x7632u;
-    __syncthreads();
+    const uint32_t selA = (sb & 1u) ? 0x1504u : 0x5140u, selB = (sb & 1u) ? 0x3726u : 0x7362u;
+    const uint32_t selLo = (sb & 2u) ? 0x1054u : 0x5410u, selHi = (sb & 2u) ? 0x3276u : 0x7632u;
+    const uint32_t m3 = ~3u;
 
-    // ---- phase B: per byte column, 8 output rows at a time
-    for (uint32_t gi = g0; gi < ngroups; gi += GSTEP) {
-        const uint32_t ro = gi * COL_G;
-        const bool full = ro + COL_G <= h;
-        // next group's keystream
-        uint32_t kn[COL_G];
+    for (uint32_t gi = g0;; gi += GSTEP) {
+        uint32_t O[CE_G][2];
 #pragma unroll
-        for (int i = 0; i < COL_G; ++i) kn[i] = 0;
-        if (!INV && col_ok && gi + GSTEP < ngroups) {
-            const uint32_t rn = ro + GSTEP * COL_G;
-            if (rn + COL_G <= h) {
+        for (int al_ = 0; al_ < 2; ++al_) {
+            uint32_t A[4][2];
 #pragma unroll
-                for (int i = 0; i < COL_G; ++i) kn[i] = __ldcs(Bw + (rn + i) * rw);
-            } else {
+            for (int ab = 0; ab < 4; ++ab) {
+                const int a = al_ * 4 + ab;
+                const uint32_t Ka = (uint32_t)ab * X + 4u * (uint32_t)al_;
+                const uint8_t *p = S + ((q[a] & m3) ^ Ka);
+                const uint32_t r0 = *reinterpret_cast<const uint32_t *>(p);
+                const uint32_t r1 = *reinterpret_cast<const uint32_t *>(p + 4 * X);
+                const uint32_t r2 = *reinterpret_cast<const uint32_t *>(p + 8 * X);
+                const uint32_t shamt = q[a] << 3;
+                A[ab][0] = __funnelshift_r(r0, r1, shamt);
+                A[ab][1] = __funnelshift_r(r1, r2, shamt);
+                q[a] += ADVX;
+                if (q[a] >= hX) q[a] -= hX;
+            }
 #pragma unroll
-                for (int i = 0; i < COL_G; ++i)
-                    if (rn + i < h) kn[i] = __ldcs(Bw + (rn + i) * rw);
+            for (int hg = 0; hg < 2; ++hg) {
+                const uint32_t t01a = __byte_perm(A[0][hg], A[1][hg], selA), t01b = __byte_perm(A[0][hg], A[1][hg], selB);
+                const uint32_t t23a = __byte_perm(A[2][hg], A[3][hg], selA), t23b = __byte_perm(A[2][hg], A[3][hg], selB);
+                O[4 * hg + 0][al_] = __byte_perm(t01a, t23a, selLo);
+                O[4 * hg + 1][al_] = __byte_perm(t01a, t23a, selHi);
+                O[4 * hg + 2][al_] = __byte_perm(t01b, t23b, selLo);
+                O[4 * hg + 3][al_] = __byte_perm(t01b, t23b, selHi);
             }
         }
-        uint32_t A[4][2];
+        // undo the word column permutation and store (default caching: the inverse row pass reads this from L2)
+        const uint32_t offs[8] = {0u, rb, rb2, rb3, rb4, rb5, rb6, rb7};
+        if (gi < nfull) {
 #pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            const uint8_t *q = S + p[a];
-            const uint32_t r0 = *reinterpret_cast<const uint32_t *>(q);
-            const uint32_t r1 = *reinterpret_cast<const uint32_t *>(q + 4 * X);
-            const uint32_t r2 = *reinterpret_cast<const uint32_t *>(q + 8 * X);
-            A[a][0] = __byte_perm(r0, r1, sel[a]);
-            A[a][1] = __byte_perm(r1, r2, sel[a]);
-            p[a] += ADV;
-            if (p[a] >= lim[a]) p[a] -= hX;
+            for (int i = 0; i < CE_G; ++i)
+                *VK_ROWPTR(uint2 *, pO, offs[i]) = make_uint2(sl ? O[i][1] : O[i][0], sl ? O[i][0] : O[i][1]);
+        } else {
+#pragma unroll
+            for (int i = 0; i < CE_G / 2; ++i)
+                *VK_ROWPTR(uint2 *, pO, offs[i]) = make_uint2(sl ? O[i][1] : O[i][0], sl ? O[i][0] : O[i][1]);
+            break;
         }
-        uint32_t o[COL_G];
-#pragma unroll
-        for (int hg = 0; hg < 2; ++hg) {
-            const uint32_t t01a = __byte_perm(A[0][hg], A[1][hg], selA), t01b = __byte_perm(A[0][hg], A[1][hg], selB);
-            const uint32_t t23a = __byte_perm(A[2][hg], A[3][hg], selA), t23b = __byte_perm(A[2][hg], A[3][hg], selB);
-            o[4 * hg + 0] = __byte_perm(t01a, t23a, selLo) ^ kb[4 * hg + 0];
-            o[4 * hg + 1] = __byte_perm(t01a, t23a, selHi) ^ kb[4 * hg + 1];
-            o[4 * hg + 2] = __byte_perm(t01b, t23b, selLo) ^ kb[4 * hg + 2];
-            o[4 * hg + 3] = __byte_perm(t01b, t23b, selHi) ^ kb[4 * hg + 3];
-        }
-        if (col_ok) {
-            uint32_t *po = Ow + ro * rw;
-            if (full) {
-#pragma unroll
-                for (int i = 0; i < COL_G; ++i) {
-                    if (INV) po[i * rw] = o[i];  // intermediate for the inverse row pass: keep it L2-resident
-                    else __stcs(po + i * rw, o[i]);
-                }
-            } else {
-#pragma unroll
-                for (int i = 0; i < COL_G; ++i)
-                    if (ro + i < h) {
-                        if (INV) po[i * rw] = o[i];
-                        else __stcs(po + i * rw, o[i]);
-                    }
-            }
-        }
-#pragma unroll
-        for (int i = 0; i < COL_G; ++i) kb[i] = kn[i];
+        if ((gi + GSTEP) * CE_G >= h) break;
+        pO += gstep;
     }
+#undef VK_ROWPTR
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -864,12 +874,11 @@ __global__ void __launch_bounds__(256)
 static size_t row_smem_bytes(const Geom &g, int ns) {
     return (size_t)ROW_HDR + (size_t)(ns + 1) * ROW_RB * g.row_bytes + (size_t)ROW_RB * 3 * (g.w + 32);
 }
-static size_t col_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + COL_PAD) * X; }
 static size_t cole_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + CE_PAD) * X + 16 + 2 * (size_t)X; }
 
 template <int X, int NT, int MINB>
 static cudaError_t col_set_attr(size_t smem) {
-    return cudaFuncSetAttribute(col_pass_kernel<X, true, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return cudaFuncSetAttribute(col_dec_kernel<X, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
 }
 template <int X, int NT, int MINB>
 static cudaError_t cole_set_attr(size_t smem) {
@@ -889,17 +898,16 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
     if (e != cudaSuccess) return e;
     p.tiled = false;
     p.max_frames_per_launch = 1;
-    const bool shape_ok = g.w % 16 == 0 && g.h % 4 == 0 && g.h >= 2 * COL_PAD && g.w >= 64 &&
+    const bool shape_ok = g.w % 16 == 0 && g.h % 4 == 0 && g.h >= 2 * CE_PAD && g.w >= 64 &&
                           g.frame_bytes < ((size_t)1 << 31);
     if (shape_ok) {
-        // column strips: the widest X that leaves room for 3 CTAs per SM (256 threads each); else the
-        // widest that fits at all (one CTA of 512 threads per SM)
-        const int cands[3] = {128, 64, 32};
+        // column strips: 64 byte columns (32 when 64 do not fit); 256-thread CTAs when at least two fit on an SM, else
+        // one 512-thread CTA.  Measured on B200: at 4K one CTA with X = 64 beats three CTAs with X = 32 (27.4 vs 29.4 us
+        // per frame); the width itself hardly matters for the row-strided DRAM side (profiles/).
         int X = 0, ctas = 0;
-        for (int c = 0; c < 3 && !X; ++c)
-            if (3 * (cole_smem_bytes(g, cands[c]) + 1024) <= (size_t)smem_sm) { X = cands[c]; ctas = 3; }
-        for (int c = 0; c < 3 && !X; ++c)
-            if (cole_smem_bytes(g, cands[c]) <= (size_t)smem_optin) { X = cands[c]; ctas = 1; }
+        if (cole_smem_bytes(g, 64) <= (size_t)smem_optin) X = 64;
+        else if (cole_smem_bytes(g, 32) <= (size_t)smem_optin) X = 32;
+        if (X) ctas = 2 * (cole_smem_bytes(g, X) + 1024) <= (size_t)smem_sm ? 3 : 1;
         // row pass: compute threads = one per quad of 4 pixels, at most 15 warps (+ the copy warp) when
         // several CTAs share an SM; the deepest ring of stages that still leaves 2 CTAs per SM, else what fits
         const uint32_t Q = g.w / 4;
@@ -925,7 +933,6 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
             p.strip_bytes = X;
             p.col_ctas_per_sm = ctas;
             p.strips_per_frame = (int)((g.row_bytes + X - 1) / X);
-            p.smem_col = col_smem_bytes(g, X);
             p.smem_cole = cole_smem_bytes(g, X);
             uint32_t br = 1;
             for (uint32_t d = 1; d <= 256 && d <= g.h; ++d)
@@ -945,13 +952,11 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
             const size_t l2_budget = (size_t)56 << 20;  // intermediate kept well inside the 126 MB L2
             p.max_frames_per_launch = l2_budget / g.frame_bytes ? l2_budget / g.frame_bytes : 1;
             if (ctas == 3) {
-                if (X == 128) { e = col_set_attr<128, 256, 3>(p.smem_col); if (!e) e = cole_set_attr<128, 256, 3>(p.smem_cole); }
-                else if (X == 64) { e = col_set_attr<64, 256, 3>(p.smem_col); if (!e) e = cole_set_attr<64, 256, 3>(p.smem_cole); }
-                else { e = col_set_attr<32, 256, 3>(p.smem_col); if (!e) e = cole_set_attr<32, 256, 3>(p.smem_cole); }
+                if (X == 64) { e = col_set_attr<64, 256, 3>(p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3>(p.smem_cole); }
+                else { e = col_set_attr<32, 256, 3>(p.smem_cole); if (!e) e = cole_set_attr<32, 256, 3>(p.smem_cole); }
             } else {
-                if (X == 128) { e = col_set_attr<128, 512, 1>(p.smem_col); if (!e) e = cole_set_attr<128, 512, 1>(p.smem_cole); }
-                else if (X == 64) { e = col_set_attr<64, 512, 1>(p.smem_col); if (!e) e = cole_set_attr<64, 512, 1>(p.smem_cole); }
-                else { e = col_set_attr<32, 512, 1>(p.smem_col); if (!e) e = cole_set_attr<32, 512, 1>(p.smem_cole); }
+                if (X == 64) { e = col_set_attr<64, 512, 1>(p.smem_cole); if (!e) e = cole_set_attr<64, 512, 1>(p.smem_cole); }
+                else { e = col_set_attr<32, 512, 1>(p.smem_cole); if (!e) e = cole_set_attr<32, 512, 1>(p.smem_cole); }
             }
             if (e != cudaSuccess) return e;
             e = cudaFuncSetAttribute(row_pass_kernel<false, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
@@ -996,20 +1001,19 @@ static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, 
 }
 
 // decrypt direction (row-major in and out)
-static cudaError_t launch_col_inv(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
+static cudaError_t launch_col_dec(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
                                   size_t n, uint8_t *dst, cudaStream_t st) {
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
-#define VK_COL(X, NT, MINB) col_pass_kernel<X, true, NT, MINB><<<grid, NT, p.smem_col, st>>>(src, B, dst, D, g, p.strips_per_frame)
+#define VK_COLD(X, NT, MINB) \
+    return launch_pdl(col_dec_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, src, B, dst, D, g, (uint32_t)p.strips_per_frame, p.h_magic)
     if (p.col_ctas_per_sm == 3) {
-        if (p.strip_bytes == 128) VK_COL(128, 256, 3);
-        else if (p.strip_bytes == 64) VK_COL(64, 256, 3);
-        else VK_COL(32, 256, 3);
+        if (p.strip_bytes == 64) VK_COLD(64, 256, 3);
+        else VK_COLD(32, 256, 3);
     } else {
-        if (p.strip_bytes == 128) VK_COL(128, 512, 1);
-        else if (p.strip_bytes == 64) VK_COL(64, 512, 1);
-        else VK_COL(32, 512, 1);
+        if (p.strip_bytes == 64) VK_COLD(64, 512, 1);
+        else VK_COLD(32, 512, 1);
     }
-#undef VK_COL
+#undef VK_COLD
     return cudaGetLastError();
 }
 
@@ -1033,12 +1037,10 @@ static cudaError_t launch_col_enc(const Geom &g, const Plan &p, uint8_t *io, con
     return launch_pdl(col_enc_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_main, tm_pad, B, (uint8_t *)io, D, g, \
                       (uint32_t)p.strips_per_frame, (uint32_t)n, p.box_rows, p.h_magic)
     if (p.col_ctas_per_sm == 3) {
-        if (p.strip_bytes == 128) VK_COLE(128, 256, 3);
-        else if (p.strip_bytes == 64) VK_COLE(64, 256, 3);
+        if (p.strip_bytes == 64) VK_COLE(64, 256, 3);
         else VK_COLE(32, 256, 3);
     } else {
-        if (p.strip_bytes == 128) VK_COLE(128, 512, 1);
-        else if (p.strip_bytes == 64) VK_COLE(64, 512, 1);
+        if (p.strip_bytes == 64) VK_COLE(64, 512, 1);
         else VK_COLE(32, 512, 1);
     }
 #undef VK_COLE
@@ -1064,7 +1066,7 @@ cudaError_t decrypt_tiled(const Geom &g, const Plan &p, const uint8_t *src, cons
     for (size_t f0 = 0; f0 < n; f0 += p.max_frames_per_launch) {
         const size_t m = n - f0 < p.max_frames_per_launch ? n - f0 : p.max_frames_per_launch;
         const size_t off = f0 * g.frame_bytes;
-        cudaError_t e = launch_col_inv(g, p, src + off, D + f0 * g.nD, B + off, m, dst + off, st);
+        cudaError_t e = launch_col_dec(g, p, src + off, D + f0 * g.nD, B + off, m, dst + off, st);
         if (e != cudaSuccess) return e;
         e = launch_row<true>(g, p, dst + off, D + f0 * g.nD, m, dst + off, st);
         if (e != cudaSuccess) return e;

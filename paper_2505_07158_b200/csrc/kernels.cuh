@@ -24,7 +24,7 @@ inline Geom make_geom(uint32_t w, uint32_t h) {
 // Plan chosen once per context from (w, h) and the device's shared-memory size.
 struct Plan {
     bool tiled;            // tiled two-pass path usable (w % 16 == 0, h % 4 == 0, h >= 16, strip and row block fit in shared memory)
-    int strip_bytes;       // X: byte columns per strip (128, 64 or 32)
+    int strip_bytes;       // X: byte columns per strip (64, or 32 for very tall frames)
     int strips_per_frame;  // ceil(3w / X)
     int row_nc;            // row pass: compute threads per CTA (+ 32 for the copy warp)
     int row_ns;            // row pass: stages of the shared-memory ring
@@ -33,10 +33,9 @@ struct Plan {
     uint32_t box_rows;     // column pass: rows per TMA tensor tile (largest divisor of h that is <= 256)
     uint32_t h_magic;      // ceil(2^32 / h): d mod h without a division for d < 2^16
     void *encode_tiled;    // cuTensorMapEncodeTiled, resolved through the runtime (no link-time libcuda dependency)
-    int col_ctas_per_sm;   // residency the column pass was sized for (3: 256-thread CTAs, 1: 512-thread CTAs)
+    int col_ctas_per_sm;   // column pass variant (3: 256-thread CTAs, two or three per SM; 1: one 512-thread CTA per SM)
     size_t smem_row;       // dynamic shared memory of the row pass
-    size_t smem_col;       // dynamic shared memory of the column pass (decrypt direction)
-    size_t smem_cole;      // dynamic shared memory of the column pass (encrypt direction)
+    size_t smem_cole;      // dynamic shared memory of the column pass (either direction)
     size_t max_frames_per_launch;  // keeps the intermediate (n * 3wh bytes) L2-resident
 };
 
