@@ -146,6 +146,15 @@ int vcrypt_launch_count(const vcrypt_ctx *ctx, uint64_t *last_call, uint64_t *to
  * (The paper's Fig. 13 phase split.) */
 int vcrypt_last_stage_ms(const vcrypt_ctx *ctx, double out[4]);
 
+/* Memory-system probe (bench hook): moves the bytes of one vcrypt_encrypt_device call on `frames` frames of this
+ * context's shape with no cipher arithmetic, `reps` times on the context's device, and returns the mean time of
+ * one repetition in microseconds (CUDA events).  which = 0: sequential copy (read 3wh + write 3wh per frame);
+ * 1: the traffic of any two-pass design, sequential (pass 1 reads F and writes an L2-resident intermediate,
+ * pass 2 reads it back, reads B, writes the result: 5 trips through L2 per byte; cf. DESIGN.md "What bounds the
+ * path"); 2: read B + write result in 64-byte-wide column strips (the DRAM side of the column pass).
+ * Allocates and frees about 3.6 GB of device memory.  VCRYPT_E_ARG for a bad `which`, frames = 0 or reps < 1. */
+int vcrypt_memory_probe(vcrypt_ctx *ctx, int which, size_t frames, int reps, double *us_per_rep);
+
 #ifdef __cplusplus
 }
 #endif

@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
     L.vcrypt_decrypt_device.argtypes = [_vp, _vp, _vp, _vp, C.c_size_t, _vp, _vp]
     L.vcrypt_launch_count.argtypes = [_vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.vcrypt_last_stage_ms.argtypes = [_vp, C.POINTER(C.c_double)]
+    L.vcrypt_memory_probe.argtypes = [_vp, C.c_int, C.c_size_t, C.c_int, C.POINTER(C.c_double)]
     _lib = L
     return L
 
@@ -211,6 +212,12 @@ class Vcrypt:
         a, b = C.c_uint64(), C.c_uint64()
         self._check(self.L.vcrypt_launch_count(self._p, C.byref(a), C.byref(b)), "vcrypt_launch_count")
         return int(a.value), int(b.value)
+
+    def memory_probe(self, which: int, frames: int, reps: int = 20) -> float:
+        """vcrypt_memory_probe: microseconds per repetition (0 sequential copy, 1 two-pass traffic, 2 column strips)."""
+        us = C.c_double()
+        self._check(self.L.vcrypt_memory_probe(self._p, which, frames, reps, C.byref(us)), "vcrypt_memory_probe")
+        return float(us.value)
 
     def last_stage_ms(self):
         out = (C.c_double * 4)()

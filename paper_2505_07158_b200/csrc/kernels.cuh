@@ -56,4 +56,7 @@ cudaError_t encrypt_generic(const Geom &g, const uint8_t *src, const uint16_t *D
 cudaError_t decrypt_generic(const Geom &g, const uint8_t *src, const uint16_t *D, const uint8_t *B, size_t n,
                             uint8_t *dst, cudaStream_t st, int *launches);
 
+// Memory-system probes (membench.cu): see vcrypt_memory_probe in include/vcrypt.h.
+cudaError_t memory_probe(const Geom &g, int which, size_t frames, int reps, cudaStream_t st, double *us_per_call);
+
 }  // namespace vk

@@ -415,6 +415,17 @@ extern "C" int vcrypt_decrypt_device(vcrypt_ctx *c, const void *d_cipher, const 
     return device_call(c, true, d_cipher, d_D, d_B, n, d_plain, stream);
 }
 
+extern "C" int vcrypt_memory_probe(vcrypt_ctx *c, int which, size_t frames, int reps, double *us_per_rep) {
+    if (!c || !us_per_rep || which < 0 || which > 2 || frames == 0 || reps < 1) return VCRYPT_E_ARG;
+    if (!c->cuda) return VCRYPT_E_CUDA;
+    VC_CUDA(c, cudaSetDevice(c->device));
+    const cudaError_t e = vk::memory_probe(c->g, which, frames, reps, nullptr, us_per_rep);
+    if (e == cudaErrorInvalidValue) return VCRYPT_E_ARG;
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return VCRYPT_E_NOMEM; }
+    if (e != cudaSuccess) return cuda_fail(c, e, "memory probe");
+    return VCRYPT_OK;
+}
+
 // =====================================================================================================
 // host-buffer pipeline: Algorithm 1's loop over frames, batched and overlapped
 // =====================================================================================================

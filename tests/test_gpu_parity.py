@@ -69,8 +69,12 @@ def oracle_frames(orc, F, D, B, inverse=False):
     return np.stack([orc.confuse_xor(F[k], D[k], B[k], inverse=inverse) for k in range(F.shape[0])])
 
 
-# shapes on the tiled path (w % 16 == 0): several column strips, ragged last strip, several row blocks
-TILED = [(256, 256, 1), (64, 48, 3), (16, 1, 2), (16, 5, 1), (48, 33, 2), (640, 480, 2), (80, 7, 4), (1008, 19, 1)]
+# shapes on the tiled path (w % 16 == 0, w >= 64, h % 4 == 0, h >= 16): several column strips, a ragged last strip
+# (3w % 64 != 0: TMA out-of-bounds columns), h % 8 == 4 (half row group at the bottom), h not a multiple of the TMA
+# tile height, a single 4-row block per CTA, more quads than compute threads (w = 2048); and w % 16 == 0 shapes
+# that fall back to the any-shape kernels (w < 64 or h % 4 != 0)
+TILED = [(256, 256, 1), (64, 48, 3), (80, 32, 2), (112, 20, 3), (1008, 36, 1), (64, 16, 5), (2048, 24, 1), (144, 1028, 1),
+         (640, 480, 2), (16, 1, 2), (16, 5, 1), (48, 33, 2), (80, 7, 4), (1008, 19, 1)]
 # shapes only the any-shape kernels take
 RAGGED = [(1, 1, 1), (1, 7, 2), (5, 1, 1), (17, 9, 3), (33, 20, 2), (100, 37, 1), (15, 64, 1), (250, 3, 2)]
 
