@@ -117,11 +117,12 @@ def test_in_place_and_forced_generic(torch_cuda, vb, orc, w, h, nf, generic):
 
 def test_many_frames_per_call_split_into_l2_sized_launches(torch_cuda, vb, orc):
     """More frames than one L2-resident launch holds: the call splits, results unchanged."""
-    w, h, nf = 640, 480, 80  # 73.7 MB of frames
+    w, h, nf = 640, 480, 120  # 110.6 MB of frames: two launch pairs (113 + 7 frames)
     F, D, B = rnd_case(w, h, nf, seed=21)
     v = gpu_ctx(vb, w, h)
     E = run_device(torch_cuda, v, F, D, B)
-    for k in (0, 1, 37, 68, 69, 70, 79):
+    assert v.launch_count()[0] == 4
+    for k in (0, 1, 37, 112, 113, 114, 119):
         assert np.array_equal(E[k], orc.confuse_xor(F[k], D[k], B[k])), k
     assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
 
