@@ -455,6 +455,13 @@ __device__ __forceinline__ void tma_load_2d(void *smem_dst, const CUtensorMap *t
         : "memory");
 }
 
+// L2 prefetch of one tensor tile (DRAM -> L2 only; no shared memory, no completion to wait for)
+__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap *tm, int32_t x, int32_t y) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(reinterpret_cast<uint64_t>(tm)), "r"(x),
+                 "r"(y)
+                 : "memory");
+}
+
 // p + off as one IMAD.WIDE.U32 (FMA pipe) instead of a two-instruction 64-bit add on the ALU pipe
 __device__ __forceinline__ uint64_t mad_wide_ptr(const void *p, uint32_t off) {
     uint64_t r;
@@ -465,13 +472,14 @@ __device__ __forceinline__ uint64_t mad_wide_ptr(const void *p, uint32_t off) {
 template <int X, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
     col_enc_kernel(const __grid_constant__ CUtensorMap tm_main, const __grid_constant__ CUtensorMap tm_pad,
-                   const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
-                   uint32_t strips_per_frame, uint32_t nframes, uint32_t box_rows, uint32_t h_magic) {
+                   const __grid_constant__ CUtensorMap tm_B, const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
+                   uint32_t strips_per_frame, uint32_t nframes, uint32_t box_rows, uint32_t h_magic, uint32_t pf_rows) {
     extern __shared__ __align__(128) uint8_t S[];
     constexpr uint32_t LPS = X / 8;       // lanes per strip row
     constexpr uint32_t NSUB = 32 / LPS;   // sub-warps per warp
     constexpr uint32_t NW = NT / 32;
     constexpr uint32_t GSTEP = NW * NSUB;  // groups between two iterations of a sub-warp
+    constexpr uint32_t CE_AHEAD = 2u * GSTEP * CE_G;  // keystream rows on their way to L2 ahead of the CTA: two iterations (measured optimum)
     const uint32_t h = g.h, rb = g.row_bytes;
     uint64_t *bar = reinterpret_cast<uint64_t *>(S + (size_t)(h + CE_PAD) * X);
     uint16_t *ups = reinterpret_cast<uint16_t *>(S + (size_t)(h + CE_PAD) * X + 16);  // [X] source row offset per byte column
@@ -481,7 +489,11 @@ __global__ void __launch_bounds__(NT, MINB)
     const uint32_t x0 = (blockIdx.x - fr * strips_per_frame) * X;
 
     pdl_trigger();
+    // keystream look-ahead: thread 0 asks the TMA engine to pull the strip's keystream tiles into L2, CE_AHEAD rows
+    // ahead of the row group the CTA is working on (the threads' own loads then hit L2 instead of waiting on DRAM)
+    uint32_t pf_row = 0;
     if (threadIdx.x == 0) {
+        for (; pf_row < h && pf_row < CE_AHEAD; pf_row += pf_rows) tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
         mbar_init(bar, 1);
         pdl_wait();  // the strip is the row pass's output
         const uint64_t pol = policy_evict_first();
@@ -615,6 +627,9 @@ __global__ void __launch_bounds__(NT, MINB)
         // keystream of the next group
         const uint32_t gn = gi + GSTEP;
         if (gn * CE_G >= h) break;
+        if (threadIdx.x == 0)
+            for (; pf_row < h && pf_row < gn * CE_G + CE_AHEAD; pf_row += pf_rows)
+                tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
         pB += gstep;
         pO += gstep;
         if (gn < nfull) {
@@ -639,8 +654,9 @@ __global__ void __launch_bounds__(NT, MINB)
 // ---------------------------------------------------------------------------------------------
 template <int X, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
-    col_dec_kernel(const uint8_t *src, const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
-                   uint32_t strips_per_frame, uint32_t h_magic) {
+    col_dec_kernel(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ CUtensorMap tm_B, const uint8_t *src,
+                   const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
+                   uint32_t strips_per_frame, uint32_t h_magic, uint32_t box_rows) {
     extern __shared__ __align__(128) uint8_t S[];
     constexpr uint32_t LPS = X / 8;       // lanes per strip row
     constexpr uint32_t NSUB = 32 / LPS;   // sub-warps per warp
@@ -653,6 +669,15 @@ __global__ void __launch_bounds__(NT, MINB)
 
     pdl_wait();  // the ciphertext may be the previous kernel's output
     pdl_trigger();
+    // look-ahead: thread 0 asks the TMA engine to pull ciphertext and keystream tiles of the strip into L2, one iteration
+    // of rows ahead of the rows the CTA is loading (measured optimum; further ahead is slower)
+    constexpr uint32_t CD_AHEAD = 4u * (NT / 32) * (256 / X);
+    uint32_t pf_row = 0;
+    if (threadIdx.x == 0)
+        for (; pf_row < h && pf_row < CD_AHEAD; pf_row += box_rows) {
+            tma_prefetch_2d(&tm_src, (int32_t)x0, (int32_t)(f * h + pf_row));
+            tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
+        }
     // one thread per byte column of the strip: t = d_v mod h, the row offset of the column's source
     if (threadIdx.x >= NT - X) {
         const uint32_t xs = threadIdx.x - (NT - X);
@@ -699,6 +724,11 @@ __global__ void __launch_bounds__(NT, MINB)
             for (int r = 0; r < 4; ++r) { v[r] = vn[r]; k[r] = kn[r]; }
             pS += bstep;
             pB += bstep;
+            if (threadIdx.x == 0)
+                for (; pf_row < h && pf_row < 4u * (R4 + GSTEP) + CD_AHEAD; pf_row += box_rows) {
+                    tma_prefetch_2d(&tm_src, (int32_t)x0, (int32_t)(f * h + pf_row));
+                    tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
+                }
             if (R4 + GSTEP < nblk) {
 #pragma unroll
                 for (int r = 0; r < 4; ++r) {
@@ -1003,12 +1033,27 @@ static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, 
                       (uint32_t)p.row_nc);
 }
 
+// tensor map of an n*h x 3w byte matrix with tiles of X bytes x `rows` rows
+static bool make_tmap(const Plan &p, const Geom &g, const void *base, size_t n, uint32_t rows, CUtensorMap *out) {
+    const cuuint64_t dims[2] = {g.row_bytes, (cuuint64_t)n * g.h};
+    const cuuint64_t strides[1] = {g.row_bytes};
+    const cuuint32_t es[2] = {1, 1};
+    const cuuint32_t box[2] = {(cuuint32_t)p.strip_bytes, rows};
+    EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(p.encode_tiled);
+    return enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // decrypt direction (row-major in and out)
 static cudaError_t launch_col_dec(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
                                   size_t n, uint8_t *dst, cudaStream_t st) {
+    alignas(64) CUtensorMap tm_src, tm_B;
+    const uint32_t pbox = 64;  // look-ahead tile height (rows)
+    if (!make_tmap(p, g, src, n, pbox, &tm_src) || !make_tmap(p, g, B, n, pbox, &tm_B)) return cudaErrorInvalidValue;
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
-#define VK_COLD(X, NT, MINB) \
-    return launch_pdl(col_dec_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, src, B, dst, D, g, (uint32_t)p.strips_per_frame, p.h_magic)
+#define VK_COLD(X, NT, MINB)                                                                                              \
+    return launch_pdl(col_dec_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_src, tm_B, src, B, dst, D, g,           \
+                      (uint32_t)p.strips_per_frame, p.h_magic, pbox)
     if (p.col_ctas_per_sm == 3) {
         if (p.strip_bytes == 64) VK_COLD(64, 256, 3);
         else VK_COLD(32, 256, 3);
@@ -1034,11 +1079,18 @@ static cudaError_t launch_col_enc(const Geom &g, const Plan &p, uint8_t *io, con
     if (r == CUDA_SUCCESS)
         r = enc(&tm_pad, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, io, dims, strides, box_pad, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    alignas(64) CUtensorMap tm_B;
+    const uint32_t pbox = 64;  // look-ahead tile height (rows)
+    const cuuint32_t box_pf[2] = {(cuuint32_t)p.strip_bytes, pbox};
+    if (r == CUDA_SUCCESS)
+        r = enc(&tm_B, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(B), dims, strides, box_pf, es,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
 #define VK_COLE(X, NT, MINB)                                                                                        \
-    return launch_pdl(col_enc_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_main, tm_pad, B, (uint8_t *)io, D, g, \
-                      (uint32_t)p.strips_per_frame, (uint32_t)n, p.box_rows, p.h_magic)
+    return launch_pdl(col_enc_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_main, tm_pad, tm_B, B, (uint8_t *)io, D, g, \
+                      (uint32_t)p.strips_per_frame, (uint32_t)n, p.box_rows, p.h_magic, pbox)
     if (p.col_ctas_per_sm == 3) {
         if (p.strip_bytes == 64) VK_COLE(64, 256, 3);
         else VK_COLE(32, 256, 3);
