@@ -35,9 +35,9 @@ METRIC = "FHD frames/s encrypted"
 UNIT = "frames/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum of the two kernels of one encrypt call (8 FHD frames; 2 4K frames per
-# launch pair), from the ncu --set full capture summarised in profiles/r1e_ncu_full_summary.csv
-NCU_TRAFFIC_PER_CALL = {"C4": 130.66e6}  # bytes; the rest of the 149.4 MB is output still dirty in L2 when the call ends
-NCU_COL_SHARE = 0.60
+# launch pair), from the ncu --set full capture summarised in profiles/r1f_ncu_full_summary.csv
+NCU_TRAFFIC_PER_CALL = {"C4": 142.0e6}  # bytes; part of the 149.4 MB of a call is output still dirty in L2 when it ends
+NCU_COL_SHARE = 0.585
 
 
 def hbm_peak():
