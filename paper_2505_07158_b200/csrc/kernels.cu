@@ -42,47 +42,8 @@
 namespace vk {
 
 // ---------------------------------------------------------------------------------------------
-// small helpers
+// async-copy / mbarrier PTX (sm_90+; SASS: UBLKCP, UTMALDG, UTMAPF, SYNCS)
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t pick2(uint32_t wa, int ba, uint32_t wb, int bb) {
-    // byte 0 <- wa.byte[ba], byte 1 <- wb.byte[bb]
-    return __byte_perm(wa, wb, (uint32_t)(ba | ((4 + bb) << 4)));
-}
-__device__ __forceinline__ uint32_t join2(uint32_t lo, uint32_t hi) { return __byte_perm(lo, hi, 0x5410); }
-
-// 48 interleaved bytes (16 pixels, 12 words) -> three planes of 4 words
-__device__ __forceinline__ void deinterleave16(const uint32_t (&in)[12], uint32_t (&P)[3][4]) {
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            const int i0 = 3 * (4 * m) + c, i1 = i0 + 3, i2 = i0 + 6, i3 = i0 + 9;
-            P[c][m] = join2(pick2(in[i0 >> 2], i0 & 3, in[i1 >> 2], i1 & 3),
-                            pick2(in[i2 >> 2], i2 & 3, in[i3 >> 2], i3 & 3));
-        }
-}
-
-// three planes of 4 words -> 48 interleaved bytes
-__device__ __forceinline__ void interleave16(const uint32_t (&P)[3][4], uint32_t (&out)[12]) {
-#pragma unroll
-    for (int n = 0; n < 12; ++n) {
-        const int b0 = 4 * n, b1 = b0 + 1, b2 = b0 + 2, b3 = b0 + 3;  // byte b = 3*pixel + channel
-        out[n] = join2(pick2(P[b0 % 3][(b0 / 3) >> 2], (b0 / 3) & 3, P[b1 % 3][(b1 / 3) >> 2], (b1 / 3) & 3),
-                       pick2(P[b2 % 3][(b2 / 3) >> 2], (b2 / 3) & 3, P[b3 % 3][(b3 / 3) >> 2], (b3 / 3) & 3));
-    }
-}
-
-// 4 x 4 byte transpose: out[b].byte[j] = in[j].byte[b]
-__device__ __forceinline__ void transpose4x4(const uint32_t (&in)[4], uint32_t (&out)[4]) {
-    const uint32_t t01a = __byte_perm(in[0], in[1], 0x5140), t01b = __byte_perm(in[0], in[1], 0x7362);
-    const uint32_t t23a = __byte_perm(in[2], in[3], 0x5140), t23b = __byte_perm(in[2], in[3], 0x7362);
-    out[0] = __byte_perm(t01a, t23a, 0x5410);
-    out[1] = __byte_perm(t01a, t23a, 0x7632);
-    out[2] = __byte_perm(t01b, t23b, 0x5410);
-    out[3] = __byte_perm(t01b, t23b, 0x7632);
-}
-
-// ---- async-copy / mbarrier PTX (sm_90+; SASS: UBLKCP, SYNCS) -----------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
@@ -108,13 +69,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     for (uint32_t spin = 0; !mbar_try_wait(bar, parity); ++spin)
         if (spin > (1u << 24)) __trap();
 }
-// global -> shared bulk copy (16-byte aligned, size multiple of 16), completion on the mbarrier
-__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(smem_dst)),
-                 "l"(__cvta_generic_to_global(gsrc)), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
 // shared -> global bulk copy
 __device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, uint32_t bytes) {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(__cvta_generic_to_global(gdst)),
@@ -122,58 +76,8 @@ __device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, uint3
                  : "memory");
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
-__device__ __forceinline__ void bulk_wait_read_1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-// 16-byte cp.async (LDGSTS), L2 only
-__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(__cvta_generic_to_global(gsrc))
-                 : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() {
-    asm volatile("cp.async.commit_group;" ::: "memory");
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-}
-
-// Gathers four bytes, each from a register of `r` (index i*) at byte position b*, into one word.
-// All indices are compile-time constants after unrolling, so the selector arithmetic folds away:
-// 1 PRMT for <= 2 distinct registers, 2 for 3, 3 for 4.
-__device__ __forceinline__ uint32_t gather4(const uint32_t *r, int i0, int b0, int i1, int b1, int i2, int b2, int i3,
-                                            int b3) {
-    const int idx[4] = {i0, i1, i2, i3}, by[4] = {b0, b1, b2, b3};
-    int u[4] = {i0, -1, -1, -1}, nu = 1, slot[4] = {0, 0, 0, 0};
-#pragma unroll
-    for (int k = 1; k < 4; ++k) {
-        int found = -1;
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (q < nu && u[q] == idx[k]) found = q;
-        if (found < 0) { u[nu] = idx[k]; found = nu; ++nu; }
-        slot[k] = found;
-    }
-    if (nu <= 2) {
-        uint32_t sel = 0;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) sel |= (uint32_t)(by[k] + 4 * slot[k]) << (4 * k);
-        return __byte_perm(r[u[0]], r[nu > 1 ? u[1] : u[0]], sel);
-    }
-    // first PRMT: bytes living in u0 / u1 land at their final position k
-    uint32_t sel1 = 0, sel2 = 0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        if (slot[k] < 2) { sel1 |= (uint32_t)(by[k] + 4 * slot[k]) << (4 * k); sel2 |= (uint32_t)k << (4 * k); }
-        else if (slot[k] == 2) sel2 |= (uint32_t)(4 + by[k]) << (4 * k);
-    }
-    uint32_t t = __byte_perm(__byte_perm(r[u[0]], r[u[1]], sel1), r[u[2]], sel2);
-    if (nu == 4) {
-        uint32_t sel3 = 0;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) sel3 |= (uint32_t)(slot[k] == 3 ? 4 + by[k] : k) << (4 * k);
-        t = __byte_perm(t, r[u[3]], sel3);
-    }
-    return t;
-}
 
 // ---------------------------------------------------------------------------------------------
 // Row pass: horizontal bit rotation (Algorithm 4 / Eq. 2 on the rows of Algorithm 3's bit matrix,
@@ -230,24 +134,13 @@ __device__ __forceinline__ uint64_t policy_evict_first() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
-__device__ __forceinline__ uint64_t policy_evict_last() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
+// global -> shared bulk copy (16-byte aligned, size a multiple of 16) with an L2 cache hint, completion on the mbarrier
 __device__ __forceinline__ void bulk_g2s_hint(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar, uint64_t pol) {
     asm volatile(
         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
             smem_u32(smem_dst)),
         "l"(__cvta_generic_to_global(gsrc)), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
         : "memory");
-}
-__device__ __forceinline__ void bulk_s2g_hint(void *gdst, const void *smem_src, uint32_t bytes, uint64_t pol) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(
-                     __cvta_generic_to_global(gdst)),
-                 "r"(smem_u32(smem_src)), "r"(bytes), "l"(pol)
-                 : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
 __device__ __forceinline__ void bulk_wait_read_0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 

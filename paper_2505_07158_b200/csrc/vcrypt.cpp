@@ -452,6 +452,20 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
         if ((rc = ensure_slot(c, s, !in_pinned, !out_pinned)) != VCRYPT_OK) break;
         const uint8_t *src = in + b0 * fb;
         const uint8_t *hs = hashes_in ? hashes_in + 32u * b0 : nullptr;
+        if (!in_pinned) {
+            const auto t0 = clk::now();
+            const size_t chunk = (size_t)1 << 20, total = m * fb, nch = (total + chunk - 1) / chunk;
+            uint8_t *dst = s.h_F;
+            c->pool->parallel_for(nch, [&](size_t i) {
+                const size_t o = i * chunk, len = total - o < chunk ? total - o : chunk;
+                std::memcpy(dst + o, src + o, len);
+            });
+            c->stage_ms[2] += ms_since(t0);
+        }
+        // step 15, first part: the frames do not depend on the derivation, so their upload is enqueued first and runs
+        // while the host hashes and derives (it shortens the per-batch latency; the throughput is host-bound either way)
+        cudaError_t e = cudaMemcpyAsync(s.d_F, in_pinned ? src : s.h_F, m * fb, cudaMemcpyHostToDevice, s.st);
+        if (e != cudaSuccess) { rc = cuda_fail(c, e, "upload"); break; }
         if (!decrypt) {  // Algorithm 1 steps 4-6
             const auto t0 = clk::now();
             hash_frames(c, src, m, hashes_out + 32u * b0);
@@ -464,21 +478,10 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
             c->stage_ms[1] += ms_since(t0);
             if (rc != VCRYPT_OK) break;
         }
-        if (!in_pinned) {
-            const auto t0 = clk::now();
-            const size_t chunk = (size_t)1 << 20, total = m * fb, nch = (total + chunk - 1) / chunk;
-            uint8_t *dst = s.h_F;
-            c->pool->parallel_for(nch, [&](size_t i) {
-                const size_t o = i * chunk, len = total - o < chunk ? total - o : chunk;
-                std::memcpy(dst + o, src + o, len);
-            });
-            c->stage_ms[2] += ms_since(t0);
-        }
-        // steps 15-21: upload, GPU steps, download -- asynchronous on the slot's stream
+        // steps 15-21: rest of the upload, GPU steps, download -- asynchronous on the slot's stream
         uint8_t *d_res = generic ? s.d_out : s.d_F;
         uint8_t *h_res = out_pinned ? out + b0 * fb : s.h_out;
-        cudaError_t e = cudaMemcpyAsync(s.d_F, in_pinned ? src : s.h_F, m * fb, cudaMemcpyHostToDevice, s.st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(s.d_D, s.h_D, m * nD * sizeof(uint16_t), cudaMemcpyHostToDevice, s.st);
+        e = cudaMemcpyAsync(s.d_D, s.h_D, m * nD * sizeof(uint16_t), cudaMemcpyHostToDevice, s.st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(s.d_B, s.h_B, m * fb, cudaMemcpyHostToDevice, s.st);
         if (e != cudaSuccess) { rc = cuda_fail(c, e, "upload"); break; }
         if ((rc = launch_cipher(c, decrypt, s.d_F, s.d_D, s.d_B, m, d_res, s.st)) != VCRYPT_OK) break;
@@ -495,7 +498,11 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
         const int r2 = retire_slot(c, s);
         if (rc == VCRYPT_OK) rc = r2;
     }
-    if (rc != VCRYPT_OK) return rc;  // chain untouched
+    if (rc != VCRYPT_OK) {  // chain untouched; nothing of this call may still be reading the caller's buffers
+        for (Slot &s : c->slots)
+            if (s.st) cudaStreamSynchronize(s.st);
+        return rc;
+    }
     std::memcpy(c->S, S, sizeof S);
     c->frames_done += n;
     return VCRYPT_OK;

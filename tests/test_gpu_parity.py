@@ -219,21 +219,53 @@ def test_config5_4k(vb, orc):
     sampled_parity(vb, orc, cfg, 20, {0, 7, 8, 19}, pinned=True)
 
 
-def test_config4_one_bit_pairs_npcr_uaci(vb):
-    """Pin P7 on the GPU path: one flipped plaintext bit -> NPCR ~ 255/256, UACI ~ (256^2-1)/(3*256*255)
-    (Eq. 14-16; closed forms for independent uniform ciphertexts)."""
+def test_config4_one_bit_pairs_npcr_uaci(vb, torch_cuda):
+    """Pin P7 on the GPU path, config 4's 100 pairs: one flipped plaintext bit -> NPCR ~ 255/256, UACI ~
+    (256^2-1)/(3*256*255) (Eq. 14-16; closed forms for independent uniform ciphertexts), over all
+    three channels and per channel; every pair within 5 sigma, the mean within 3 sigma / sqrt(pairs)."""
+    torch = torch_cuda
     cfg = synth.CONFIGS["C4"]
-    npcr, uaci = [], []
-    for f, g, _ in synth.one_bit_pairs(cfg, 6):
-        c1, _ = gpu_ctx(vb, cfg.w, cfg.h, batch=1).encrypt_frames(f[None])
-        c2, _ = gpu_ctx(vb, cfg.w, cfg.h, batch=1).encrypt_frames(g[None])
-        a, b = c1[0].astype(np.int16), c2[0].astype(np.int16)
-        npcr.append(100.0 * np.mean(a != b))
-        uaci.append(100.0 * np.mean(np.abs(a - b)) / 255.0)
+    pairs = 100
+    npcr, uaci, npcr_c, uaci_c = [], [], [], []
+    for f, g, _ in synth.one_bit_pairs(cfg, pairs):
+        c1, _ = gpu_ctx(vb, cfg.w, cfg.h, batch=1, n_streams=1, host_threads=8).encrypt_frames(f[None])
+        c2, _ = gpu_ctx(vb, cfg.w, cfg.h, batch=1, n_streams=1, host_threads=8).encrypt_frames(g[None])
+        a = torch.from_numpy(c1[0]).cuda().to(torch.int16)
+        b = torch.from_numpy(c2[0]).cuda().to(torch.int16)
+        ne = (a != b).to(torch.float64)
+        ad = (a - b).abs().to(torch.float64)
+        npcr.append(100.0 * float(ne.mean()))
+        uaci.append(100.0 * float(ad.mean()) / 255.0)
+        npcr_c.append([100.0 * float(ne[..., c].mean()) for c in range(3)])
+        uaci_c.append([100.0 * float(ad[..., c].mean()) / 255.0 for c in range(3)])
     n = 3 * cfg.w * cfg.h
+    e_npcr, e_uaci = 100.0 * 255 / 256, 100.0 * (256 ** 2 - 1) / (3 * 256 * 255)
     s_npcr = 100.0 * np.sqrt((255 / 256) * (1 / 256) / n)
-    assert all(abs(x - 99.609375) < 5 * s_npcr for x in npcr), npcr
-    assert all(abs(x - 33.463542) < 5 * 0.0095 for x in uaci), uaci
+    # |a - b| / 255 for independent uniform bytes: E = (256^2-1)/(3*256*255), E[d^2] = (256^2-1)/6
+    var_d = (256 ** 2 - 1) / 6.0 - ((256 ** 2 - 1) / (3 * 256.0)) ** 2
+    s_uaci = 100.0 * np.sqrt(var_d / n) / 255.0
+    assert all(abs(x - e_npcr) < 5 * s_npcr for x in npcr), npcr
+    assert all(abs(x - e_uaci) < 5 * s_uaci for x in uaci), uaci
+    assert abs(np.mean(npcr) - e_npcr) < 3 * s_npcr / np.sqrt(pairs)
+    assert abs(np.mean(uaci) - e_uaci) < 3 * s_uaci / np.sqrt(pairs)
+    s3 = np.sqrt(3.0)  # a channel has a third of the bytes
+    assert all(abs(x - e_npcr) < 5 * s_npcr * s3 for row in npcr_c for x in row)
+    assert all(abs(x - e_uaci) < 5 * s_uaci * s3 for row in uaci_c for x in row)
+
+
+def test_memory_probe_hook(vb):
+    """vcrypt_memory_probe (bench hook): plausible times, argument errors."""
+    import ctypes as C
+
+    v = gpu_ctx(vb, 640, 480)
+    t_copy, t_two, t_strip = (v.memory_probe(k, 24, 5) for k in (0, 1, 2))
+    assert 0.5 < t_copy < 1000 and 0.5 < t_strip < 1000
+    assert t_two > t_copy  # five trips through L2 against two
+    us = C.c_double()
+    assert v.L.vcrypt_memory_probe(v._p, 3, 1, 1, C.byref(us)) == vb.E_ARG
+    assert v.L.vcrypt_memory_probe(v._p, 0, 0, 1, C.byref(us)) == vb.E_ARG
+    assert v.L.vcrypt_memory_probe(v._p, 0, 1, 0, C.byref(us)) == vb.E_ARG
+    assert v.L.vcrypt_memory_probe(v._p, 0, 1, 1, None) == vb.E_ARG
 
 
 def test_failed_call_leaves_chain_untouched(vb):

@@ -84,6 +84,15 @@ def test_null_arguments_and_host_only_gpu_calls():
     assert L.vcrypt_encrypt_device(v._p, C.c_void_p(256), C.c_void_p(256), C.c_void_p(256), 1, C.c_void_p(256), None) == vb.E_CUDA
 
 
+def test_memory_probe_needs_a_gpu_context():
+    import ctypes as C
+
+    v = host_ctx(64, 48, 4)
+    us = C.c_double()
+    assert v.L.vcrypt_memory_probe(v._p, 0, 1, 1, C.byref(us)) == vb.E_CUDA
+    assert v.L.vcrypt_memory_probe(None, 0, 1, 1, C.byref(us)) == vb.E_ARG
+
+
 def test_init_without_gpu_fails_loudly():
     """No CPU fallback: on a box without a CUDA device a normal context cannot be created."""
     import torch
