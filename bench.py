@@ -8,7 +8,8 @@ One "step" = one pass of the whole hot path over the clip of the chosen config (
   value : frames/s with F_o, D, B already resident in HBM -- vcrypt_encrypt_device calls only (rows a6-a10),
           timed with CUDA events on the launching stream.
   e2e   : frames/s through vcrypt_encrypt_frames with pinned HOST buffers: sub-frame SHA-256, chain, worker
-          LHCS -> D, B, H2D, kernels, D2H all inside the timed region (rows a1-a11), wall clock.
+          LHCS -> D, B (on the GPU with --derive device, the default; on the host lanes with --derive host: same
+          bytes), H2D, kernels, D2H all inside the timed region (rows a1-a11), wall clock.
   roofline : algorithmic bytes (9wh per frame + D) / CUDA-event time of the encrypt kernels vs the measured HBM peak.
   cpu_baseline : the oracle as it stands on a bounded sample, one core.
 Prints ONE JSON line (rank 0).  Under torchrun (N > 1) every rank encrypts its own clip (weak scaling, no
@@ -142,6 +143,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--frames", type=int, default=0, help="frames per step (default: the config's clip length)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--derive", default="device", choices=["host", "device"],
+                    help="where the worker systems (D, B) of the end-to-end leg run: host lanes or the GPU (same bytes)")
+    ap.add_argument("--e2e-streams", type=int, default=0, help="pipeline depth of the end-to-end leg (0: the config's)")
     args = ap.parse_args()
     cfg = synth.CONFIGS[args.config]
     if args.impl == "reference":
@@ -256,8 +260,9 @@ def main():
     ectx = None
     e2e_s = []
     for k in range(W + K):
-        ectx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams,
-                         host_threads=threads, device=local) if ectx is None else ectx
+        ectx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=cfg.batch,
+                         n_streams=args.e2e_streams or cfg.n_streams, host_threads=threads, device=local,
+                         flags=vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0) if ectx is None else ectx
         if k == W:
             barrier()
             t_e2e0 = time.perf_counter()
@@ -313,9 +318,11 @@ def main():
         "config": {"workload": workload_name(cfg), "frames_per_step": T, "ms_per_frame_kernel": kern_ms_total / K / T,
                    "l2": f"inputs larger than L2: {3 * fb * T / 1e6:.0f} MB streamed per step, no flush needed",
                    "host_threads": threads, "host_cores": ncores, "describe": vb.describe()},
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": T * (2 * fb + 2 * nD), "d2h_bytes_per_step": T * fb,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": T * ((fb + 64 * synth.N_WORKERS) if args.derive == "device" else (2 * fb + 2 * nD)),
+                "d2h_bytes_per_step": T * fb,
                 "ms_per_frame": 1e3 * e2e_total / (K * T), "ms_per_step_median": 1e3 * statistics.median(e2e_s),
-                "stage_ms_last_call": stage, "timer": "wall clock around vcrypt_encrypt_frames, pinned host in/out"},
+                "stage_ms_last_call": stage, "derive": args.derive, "n_streams": args.e2e_streams or cfg.n_streams,
+                "timer": "wall clock around vcrypt_encrypt_frames, pinned host in/out"},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": NCU_TRAFFIC_PER_CALL.get(cfg.name),

@@ -58,6 +58,8 @@ extern "C" {
 #define VCRYPT_FLAG_HOST_ONLY 1u      /* no CUDA: host derivation hooks only (tests on CPU boxes)  */
 #define VCRYPT_FLAG_FORCE_GENERIC 2u  /* always take the any-shape gather kernels (test hook)     */
 #define VCRYPT_FLAG_HOST_SCALAR 4u    /* host derivation without SHA-NI / AVX lanes (test hook)   */
+#define VCRYPT_FLAG_DEVICE_DERIVE 8u  /* worker systems -> D, B on the GPU (same bytes): the host only
+                                         hashes and runs the serial LHCS_m chain; D and B never cross PCIe */
 
 typedef struct vcrypt_ctx vcrypt_ctx; /* opaque: chain state, host thread pool, streams, device and pinned buffers */
 
@@ -145,6 +147,13 @@ int vcrypt_launch_count(const vcrypt_ctx *ctx, uint64_t *last_call, uint64_t *to
  * over its batches: [0] hashing, [1] chain + derivation, [2] staging copies on the host, [3] waiting for the GPU.
  * (The paper's Fig. 13 phase split.) */
 int vcrypt_last_stage_ms(const vcrypt_ctx *ctx, double out[4]);
+
+/* Algorithm 1 steps 7-14 + Algorithm 2 steps 5-10 for one frame with the worker systems on the GPU (PAPER.md:85,
+ * :88-110; same bytes as vcrypt_derive): the host reconstructs the initial values with `hash` and runs LHCS_m, the
+ * device derives d_D (device, 3(H+W) uint16) and d_B (device, H x W x 3, 8-byte aligned) on `cuda_stream`.
+ * Synchronises the stream before returning (test hook); VCRYPT_E_STATE if a chaotic state became non-finite.
+ * Advances the chain by one frame on success. */
+int vcrypt_derive_device(vcrypt_ctx *ctx, const uint8_t *hash, void *d_D, void *d_B, void *cuda_stream);
 
 /* Memory-system probe (bench hook): moves the bytes of one vcrypt_encrypt_device call on `frames` frames of this
  * context's shape with no cipher arithmetic, `reps` times on the context's device, and returns the mean time of

@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 OK, E_ARG, E_KEY, E_SHAPE, E_CUDA, E_NOMEM, E_STATE = 0, -1, -2, -3, -4, -5, -6
-FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR = 1, 2, 4
+FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR, FLAG_DEVICE_DERIVE = 1, 2, 4, 8
 
 
 class Params(C.Structure):
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
     L.vcrypt_decrypt_device.argtypes = [_vp, _vp, _vp, _vp, C.c_size_t, _vp, _vp]
     L.vcrypt_launch_count.argtypes = [_vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.vcrypt_last_stage_ms.argtypes = [_vp, C.POINTER(C.c_double)]
+    L.vcrypt_derive_device.argtypes = [_vp, _vp, _vp, _vp, _vp]
     L.vcrypt_memory_probe.argtypes = [_vp, C.c_int, C.c_size_t, C.c_int, C.POINTER(C.c_double)]
     _lib = L
     return L
@@ -175,6 +176,15 @@ class Vcrypt:
         self._check(self.L.vcrypt_derive(self._p, H.ctypes.data, _host_ptr(D_out, np.uint16, 2 * self.nD, "D_out"),
                                          _host_ptr(B_out, np.uint8, self.frame_bytes, "B_out")), "vcrypt_derive")
         return D_out, B_out
+
+    def derive_device(self, hash32: bytes, d_D, d_B, stream=None):
+        """vcrypt_derive_device: D (int16/uint16 tensor, 3(h+w)) and B (uint8, h x w x 3) derived on the GPU into device tensors."""
+        H = np.frombuffer(bytes(hash32), np.uint8).copy()
+        if H.size != 32:
+            raise ValueError("hash must be 32 bytes")
+        st = 0 if stream is None else int(stream)
+        self._check(self.L.vcrypt_derive_device(self._p, H.ctypes.data, _dev_ptr(d_D, 2 * self.nD, "d_D"),
+                                                _dev_ptr(d_B, self.frame_bytes, "d_B"), st), "vcrypt_derive_device")
 
     def get_state(self):
         s = (C.c_double * 4)()

@@ -21,7 +21,8 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 CXX_FLAGS = ["-O3", "-std=c++17", "-fPIC", "-ffp-contract=off", "-fno-fast-math", "-Wall", "-Wextra",
              "-fvisibility=hidden", f"-I{CUDA_HOME}/include"]
-CU_SOURCES = ["kernels.cu", "membench.cu"]
+# (source, extra flags); derive.cu holds the chaotic-map arithmetic: no FMA contraction
+CU_SOURCES = [("kernels.cu", []), ("membench.cu", []), ("derive.cu", ["-fmad=false"])]
 # (source, extra flags)
 CXX_SOURCES = [
     ("vcrypt.cpp", []),
@@ -60,10 +61,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     hdrs = [os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
     log: list[str] = []
     objs = []
-    for name in CU_SOURCES:
+    for name, extra in CU_SOURCES:
         cu, cu_o = os.path.join(CSRC, name), os.path.join(OBJ, name.replace(".cu", ".o"))
         if force or _stale(cu_o, [cu] + hdrs):
-            _run([_nvcc(), *NVCC_FLAGS, "-c", cu, "-o", cu_o], log)
+            _run([_nvcc(), *NVCC_FLAGS, *extra, "-c", cu, "-o", cu_o], log)
         objs.append(cu_o)
     for src, extra in CXX_SOURCES:
         s, o = os.path.join(CSRC, src), os.path.join(OBJ, src.replace(".cpp", ".o"))

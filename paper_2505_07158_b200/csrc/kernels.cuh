@@ -56,6 +56,11 @@ cudaError_t encrypt_generic(const Geom &g, const uint8_t *src, const uint16_t *D
 cudaError_t decrypt_generic(const Geom &g, const uint8_t *src, const uint16_t *D, const uint8_t *B, size_t n,
                             uint8_t *dst, cudaStream_t st, int *launches);
 
+// Device-side worker systems (derive.cu): D and B of m frames from their LHCS_m records IR (m x 2n x 4 doubles, device),
+// written straight into device buffers.  *d_status gets bit 0 set if a chaotic state became non-finite.
+cudaError_t derive_device(const Geom &g, const double *d_IR, double gamma, uint32_t n, size_t m, uint16_t *d_D, uint8_t *d_B,
+                          uint32_t *d_status, cudaStream_t st);
+
 // Memory-system probes (membench.cu): see vcrypt_memory_probe in include/vcrypt.h.
 cudaError_t memory_probe(const Geom &g, int which, size_t frames, int reps, cudaStream_t st, double *us_per_call);
 

@@ -38,6 +38,10 @@ struct Slot {
     // device
     uint8_t *d_F = nullptr, *d_B = nullptr, *d_out = nullptr;  // d_out only on the any-shape kernel path
     uint16_t *d_D = nullptr;
+    // device-side derivation (VCRYPT_FLAG_DEVICE_DERIVE): LHCS_m records up, status word down
+    double *h_IR = nullptr, *d_IR = nullptr;
+    uint32_t *h_status = nullptr, *d_status = nullptr;
+    bool status_pending = false;
     // work in flight
     bool busy = false;
     uint8_t *user_out = nullptr;  // where h_out goes once `done` fires (nullptr: D2H went straight to the caller)
@@ -103,6 +107,10 @@ void free_slot(Slot &s) {
     if (s.d_B) cudaFree(s.d_B);
     if (s.d_out) cudaFree(s.d_out);
     if (s.d_D) cudaFree(s.d_D);
+    if (s.h_IR) cudaFreeHost(s.h_IR);
+    if (s.d_IR) cudaFree(s.d_IR);
+    if (s.h_status) cudaFreeHost(s.h_status);
+    if (s.d_status) cudaFree(s.d_status);
     if (s.done) cudaEventDestroy(s.done);
     if (s.st) cudaStreamDestroy(s.st);
     s = Slot{};
@@ -119,8 +127,16 @@ int ensure_slot(vcrypt_ctx *c, Slot &s, bool need_hF, bool need_hout) {
     const bool generic = !c->plan.tiled || (c->p.flags & VCRYPT_FLAG_FORCE_GENERIC);
     if (generic && !s.d_out) VC_CUDA(c, cudaMalloc(&s.d_out, fb));
     if (!s.d_D) VC_CUDA(c, cudaMalloc(&s.d_D, db));
-    if (!s.h_B) VC_CUDA(c, cudaHostAlloc(&s.h_B, fb, cudaHostAllocDefault));
-    if (!s.h_D) VC_CUDA(c, cudaHostAlloc(&s.h_D, db, cudaHostAllocDefault));
+    if (c->p.flags & VCRYPT_FLAG_DEVICE_DERIVE) {
+        const size_t irb = c->batch * 2u * (size_t)c->p.n_workers * 4u * sizeof(double);
+        if (!s.h_IR) VC_CUDA(c, cudaHostAlloc(&s.h_IR, irb, cudaHostAllocDefault));
+        if (!s.d_IR) VC_CUDA(c, cudaMalloc(&s.d_IR, irb));
+        if (!s.h_status) VC_CUDA(c, cudaHostAlloc(&s.h_status, sizeof(uint32_t), cudaHostAllocDefault));
+        if (!s.d_status) VC_CUDA(c, cudaMalloc(&s.d_status, sizeof(uint32_t)));
+    } else {
+        if (!s.h_B) VC_CUDA(c, cudaHostAlloc(&s.h_B, fb, cudaHostAllocDefault));
+        if (!s.h_D) VC_CUDA(c, cudaHostAlloc(&s.h_D, db, cudaHostAllocDefault));
+    }
     if (need_hF && !s.h_F) VC_CUDA(c, cudaHostAlloc(&s.h_F, fb, cudaHostAllocDefault));
     if (need_hout && !s.h_out) VC_CUDA(c, cudaHostAlloc(&s.h_out, fb, cudaHostAllocDefault));
     return VCRYPT_OK;
@@ -133,6 +149,10 @@ int retire_slot(vcrypt_ctx *c, Slot &s) {
     VC_CUDA(c, cudaEventSynchronize(s.done));
     c->stage_ms[3] += ms_since(t0);
     s.busy = false;
+    if (s.status_pending) {
+        s.status_pending = false;
+        if (*s.h_status) return VCRYPT_E_STATE;  // a worker system left the finite range (Q17)
+    }
     if (s.user_out) {
         const auto t1 = clk::now();
         const size_t chunk = (size_t)1 << 20, nch = (s.out_bytes + chunk - 1) / chunk;
@@ -366,6 +386,14 @@ int derive_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, u
     return ok.load() ? VCRYPT_OK : VCRYPT_E_STATE;
 }
 
+// The serial part only (Algorithm 1 steps 7-13): IR of m frames, frame after frame, into `IR` (m x 2n x 4 doubles).
+int chain_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, double *IR) {
+    const uint32_t n = c->p.n_workers;
+    for (size_t f = 0; f < m; ++f)
+        if (!vh::chain_step(S, c->p.gamma, n, hashes + 32u * f, IR + f * 2u * n * 4u)) return VCRYPT_E_STATE;
+    return VCRYPT_OK;
+}
+
 }  // namespace
 
 extern "C" int vcrypt_frame_hash(vcrypt_ctx *c, const uint8_t *frame, uint8_t *H_out) {
@@ -380,6 +408,38 @@ extern "C" int vcrypt_derive(vcrypt_ctx *c, const uint8_t *hash, uint16_t *D_out
     std::memcpy(S, c->S, sizeof S);
     const int rc = derive_frames(c, S, hash, 1, D_out, B_out);
     if (rc != VCRYPT_OK) return rc;
+    std::memcpy(c->S, S, sizeof S);
+    c->frames_done += 1;
+    return VCRYPT_OK;
+}
+
+extern "C" int vcrypt_derive_device(vcrypt_ctx *c, const uint8_t *hash, void *d_D, void *d_B, void *stream) {
+    if (!c || !hash || !d_D || !d_B) return VCRYPT_E_ARG;
+    if (!c->cuda) return VCRYPT_E_CUDA;
+    if ((((uintptr_t)d_B) & 7u) || (((uintptr_t)d_D) & 1u)) return VCRYPT_E_ARG;
+    VC_CUDA(c, cudaSetDevice(c->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t irb = 2u * (size_t)c->p.n_workers * 4u * sizeof(double);
+    double S[4];
+    std::memcpy(S, c->S, sizeof S);
+    std::vector<double> IR(2u * (size_t)c->p.n_workers * 4u);
+    int rc = chain_frames(c, S, hash, 1, IR.data());
+    if (rc != VCRYPT_OK) return rc;
+    double *d_IR = nullptr;
+    uint32_t *d_status = nullptr, h_status = 0;
+    cudaError_t e = cudaMalloc(&d_IR, irb);
+    if (e == cudaSuccess) e = cudaMalloc(&d_status, sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_IR, IR.data(), irb, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_status, 0, sizeof(uint32_t), st);
+    if (e == cudaSuccess)
+        e = vk::derive_device(c->g, d_IR, c->p.gamma, c->p.n_workers, 1, static_cast<uint16_t *>(d_D), static_cast<uint8_t *>(d_B),
+                              d_status, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_status, d_status, sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (d_IR) cudaFree(d_IR);
+    if (d_status) cudaFree(d_status);
+    if (e != cudaSuccess) return cuda_fail(c, e, "device derivation");
+    if (h_status) return VCRYPT_E_STATE;
     std::memcpy(c->S, S, sizeof S);
     c->frames_done += 1;
     return VCRYPT_OK;
@@ -472,17 +532,26 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
             hs = hashes_out + 32u * b0;
             c->stage_ms[0] += ms_since(t0);
         }
+        const bool dev_derive = (c->p.flags & VCRYPT_FLAG_DEVICE_DERIVE) != 0;
         {  // steps 7-14
             const auto t0 = clk::now();
-            rc = derive_frames(c, S, hs, m, s.h_D, s.h_B);
+            rc = dev_derive ? chain_frames(c, S, hs, m, s.h_IR) : derive_frames(c, S, hs, m, s.h_D, s.h_B);
             c->stage_ms[1] += ms_since(t0);
             if (rc != VCRYPT_OK) break;
         }
         // steps 15-21: rest of the upload, GPU steps, download -- asynchronous on the slot's stream
         uint8_t *d_res = generic ? s.d_out : s.d_F;
         uint8_t *h_res = out_pinned ? out + b0 * fb : s.h_out;
-        e = cudaMemcpyAsync(s.d_D, s.h_D, m * nD * sizeof(uint16_t), cudaMemcpyHostToDevice, s.st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(s.d_B, s.h_B, m * fb, cudaMemcpyHostToDevice, s.st);
+        if (dev_derive) {  // the worker systems run on the GPU: only the LHCS_m records go up (2n x 32 bytes per frame)
+            e = cudaMemcpyAsync(s.d_IR, s.h_IR, m * 2u * (size_t)c->p.n_workers * 4u * sizeof(double), cudaMemcpyHostToDevice, s.st);
+            if (e == cudaSuccess) e = cudaMemsetAsync(s.d_status, 0, sizeof(uint32_t), s.st);
+            if (e == cudaSuccess) e = vk::derive_device(c->g, s.d_IR, c->p.gamma, c->p.n_workers, m, s.d_D, s.d_B, s.d_status, s.st);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(s.h_status, s.d_status, sizeof(uint32_t), cudaMemcpyDeviceToHost, s.st);
+            if (e == cudaSuccess) { s.status_pending = true; c->launches_last += 1; c->launches_total += 1; }
+        } else {
+            e = cudaMemcpyAsync(s.d_D, s.h_D, m * nD * sizeof(uint16_t), cudaMemcpyHostToDevice, s.st);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(s.d_B, s.h_B, m * fb, cudaMemcpyHostToDevice, s.st);
+        }
         if (e != cudaSuccess) { rc = cuda_fail(c, e, "upload"); break; }
         if ((rc = launch_cipher(c, decrypt, s.d_F, s.d_D, s.d_B, m, d_res, s.st)) != VCRYPT_OK) break;
         e = cudaMemcpyAsync(h_res, d_res, m * fb, cudaMemcpyDeviceToHost, s.st);

@@ -253,6 +253,47 @@ def test_config4_one_bit_pairs_npcr_uaci(vb, torch_cuda):
     assert all(abs(x - e_uaci) < 5 * s_uaci * s3 for row in uaci_c for x in row)
 
 
+@pytest.mark.parametrize("w,h,n", [(64, 48, 32), (64, 48, 1), (17, 9, 3), (80, 32, 7), (256, 256, 32), (33, 5, 8), (640, 480, 6)])
+def test_device_derivation_matches_oracle(torch_cuda, vb, orc, w, h, n):
+    """NEXT-1: the worker systems on the GPU give the oracle's D and B bit for bit (fp64 RK4 without FMA
+    contraction), over ragged worker slices (n not dividing h or 3(h+w), empty bands when n > h), and keep the chain in
+    step with the host derivation."""
+    torch = torch_cuda
+    v = gpu_ctx(vb, w, h, n=n)
+    vh = gpu_ctx(vb, w, h, n=n)
+    oc = orc.ctx(synth.KEY, synth.GAMMA, n, w, h)
+    dD = torch.zeros(3 * (h + w), dtype=torch.int16, device="cuda")
+    dB = torch.zeros((h, w, 3), dtype=torch.uint8, device="cuda")
+    rng = np.random.default_rng(w + h + n)
+    for _ in range(3):  # three chained frames
+        H = rng.integers(0, 256, 32, dtype=np.uint8).tobytes()
+        D_or, B_or = oc.derive(H)
+        v.derive_device(H, dD, dB)
+        assert np.array_equal(dD.cpu().numpy().view(np.uint16), D_or)
+        assert np.array_equal(dB.cpu().numpy(), B_or)
+        vh.derive(H)
+        assert np.array_equal(v.get_state()[0], vh.get_state()[0]) and v.get_state()[1] == vh.get_state()[1]
+
+
+@pytest.mark.parametrize("cfgname,nframes", [("C1", 1), ("C2", 24), ("C4", 20)])
+def test_whole_path_with_device_derivation(vb, orc, cfgname, nframes):
+    """vcrypt_encrypt_frames / vcrypt_decrypt_frames with VCRYPT_FLAG_DEVICE_DERIVE: same ciphertext, hashes and plaintext."""
+    cfg = synth.CONFIGS[cfgname]
+    frames = synth.video(cfg, nframes)
+    enc = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams, flags=vb.FLAG_DEVICE_DERIVE)
+    C, Hs = enc.encrypt_frames(frames)
+    ref = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
+    C2, H2 = ref.encrypt_frames(frames)
+    assert np.array_equal(Hs, H2) and np.array_equal(C, C2)
+    oc = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    k = min(2, nframes)
+    Co, Ho = oc.encrypt_frames(frames[:k])
+    assert np.array_equal(C[:k], Co) and np.array_equal(Hs[:k], Ho)
+    dec = gpu_ctx(vb, cfg.w, cfg.h, batch=3, n_streams=2, flags=vb.FLAG_DEVICE_DERIVE)
+    assert np.array_equal(dec.decrypt_frames(C, Hs), frames)
+    assert enc.get_state()[1] == nframes and np.array_equal(enc.get_state()[0], ref.get_state()[0])
+
+
 def test_memory_probe_hook(vb):
     """vcrypt_memory_probe (bench hook): plausible times, argument errors."""
     import ctypes as C
