@@ -145,6 +145,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--derive", default="device", choices=["host", "device"],
                     help="where the worker systems (D, B) of the end-to-end leg run: host lanes or the GPU (same bytes)")
+    ap.add_argument("--hash", default="host", choices=["host", "device"],
+                    help="where the sub-frame SHA-256 of the end-to-end leg runs (same H)")
+    ap.add_argument("--e2e-batch", type=int, default=0, help="frames per pipeline slot of the end-to-end leg (0: the config's)")
     ap.add_argument("--e2e-streams", type=int, default=0, help="pipeline depth of the end-to-end leg (0: the config's)")
     args = ap.parse_args()
     cfg = synth.CONFIGS[args.config]
@@ -260,9 +263,10 @@ def main():
     ectx = None
     e2e_s = []
     for k in range(W + K):
-        ectx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=cfg.batch,
+        ectx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=args.e2e_batch or cfg.batch,
                          n_streams=args.e2e_streams or cfg.n_streams, host_threads=threads, device=local,
-                         flags=vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0) if ectx is None else ectx
+                         flags=(vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0) |
+                         (vb.FLAG_DEVICE_HASH if args.hash == "device" else 0)) if ectx is None else ectx
         if k == W:
             barrier()
             t_e2e0 = time.perf_counter()
@@ -321,7 +325,7 @@ def main():
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": T * ((fb + 64 * synth.N_WORKERS) if args.derive == "device" else (2 * fb + 2 * nD)),
                 "d2h_bytes_per_step": T * fb,
                 "ms_per_frame": 1e3 * e2e_total / (K * T), "ms_per_step_median": 1e3 * statistics.median(e2e_s),
-                "stage_ms_last_call": stage, "derive": args.derive, "n_streams": args.e2e_streams or cfg.n_streams,
+                "stage_ms_last_call": stage, "derive": args.derive, "hash": args.hash, "batch": args.e2e_batch or cfg.batch, "n_streams": args.e2e_streams or cfg.n_streams,
                 "timer": "wall clock around vcrypt_encrypt_frames, pinned host in/out"},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

@@ -60,6 +60,8 @@ extern "C" {
 #define VCRYPT_FLAG_HOST_SCALAR 4u    /* host derivation without SHA-NI / AVX lanes (test hook)   */
 #define VCRYPT_FLAG_DEVICE_DERIVE 8u  /* worker systems -> D, B on the GPU (same bytes): the host only
                                          hashes and runs the serial LHCS_m chain; D and B never cross PCIe */
+#define VCRYPT_FLAG_DEVICE_HASH 16u   /* sub-frame SHA-256 of vcrypt_encrypt_frames on the GPU, on the frames it
+                                         uploads anyway (same H); shapes with 3W % 16 != 0 are hashed on the host */
 
 typedef struct vcrypt_ctx vcrypt_ctx; /* opaque: chain state, host thread pool, streams, device and pinned buffers */
 
@@ -147,6 +149,11 @@ int vcrypt_launch_count(const vcrypt_ctx *ctx, uint64_t *last_call, uint64_t *to
  * over its batches: [0] hashing, [1] chain + derivation, [2] staging copies on the host, [3] waiting for the GPU.
  * (The paper's Fig. 13 phase split.) */
 int vcrypt_last_stage_ms(const vcrypt_ctx *ctx, double out[4]);
+
+/* H of n frames resident in device memory, hashed on the GPU: one thread per (frame, row band), the band
+ * digests xor-ed per frame.  d_frames: device, n x H x W x 3, 16-byte aligned; hashes_out: host, n x 32.  Needs
+ * 3W % 16 == 0 (VCRYPT_E_SHAPE otherwise).  Synchronises the stream before returning (test hook); does not touch the chain. */
+int vcrypt_frame_hash_device(vcrypt_ctx *ctx, const void *d_frames, size_t n, uint8_t *hashes_out, void *cuda_stream);
 
 /* Algorithm 1 steps 7-14 + Algorithm 2 steps 5-10 for one frame with the worker systems on the GPU (PAPER.md:85,
  * :88-110; same bytes as vcrypt_derive): the host reconstructs the initial values with `hash` and runs LHCS_m, the

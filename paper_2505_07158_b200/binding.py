@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 OK, E_ARG, E_KEY, E_SHAPE, E_CUDA, E_NOMEM, E_STATE = 0, -1, -2, -3, -4, -5, -6
-FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR, FLAG_DEVICE_DERIVE = 1, 2, 4, 8
+FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR, FLAG_DEVICE_DERIVE, FLAG_DEVICE_HASH = 1, 2, 4, 8, 16
 
 
 class Params(C.Structure):
@@ -66,6 +66,7 @@ def lib() -> C.CDLL:
     L.vcrypt_launch_count.argtypes = [_vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.vcrypt_last_stage_ms.argtypes = [_vp, C.POINTER(C.c_double)]
     L.vcrypt_derive_device.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    L.vcrypt_frame_hash_device.argtypes = [_vp, _vp, C.c_size_t, _vp, _vp]
     L.vcrypt_memory_probe.argtypes = [_vp, C.c_int, C.c_size_t, C.c_int, C.POINTER(C.c_double)]
     _lib = L
     return L
@@ -176,6 +177,15 @@ class Vcrypt:
         self._check(self.L.vcrypt_derive(self._p, H.ctypes.data, _host_ptr(D_out, np.uint16, 2 * self.nD, "D_out"),
                                          _host_ptr(B_out, np.uint8, self.frame_bytes, "B_out")), "vcrypt_derive")
         return D_out, B_out
+
+    def frame_hash_device(self, d_frames, stream=None) -> np.ndarray:
+        """vcrypt_frame_hash_device: H of the frames of a CUDA tensor (n, h, w, 3), hashed on the GPU -> (n, 32) uint8."""
+        n = int(d_frames.shape[0])
+        out = np.empty((n, 32), np.uint8)
+        st = 0 if stream is None else int(stream)
+        self._check(self.L.vcrypt_frame_hash_device(self._p, _dev_ptr(d_frames, n * self.frame_bytes, "d_frames"), n,
+                                                    out.ctypes.data, st), "vcrypt_frame_hash_device")
+        return out
 
     def derive_device(self, hash32: bytes, d_D, d_B, stream=None):
         """vcrypt_derive_device: D (int16/uint16 tensor, 3(h+w)) and B (uint8, h x w x 3) derived on the GPU into device tensors."""

@@ -42,6 +42,10 @@ struct Slot {
     double *h_IR = nullptr, *d_IR = nullptr;
     uint32_t *h_status = nullptr, *d_status = nullptr;
     bool status_pending = false;
+    // device-side hashing (VCRYPT_FLAG_DEVICE_HASH): H of the batch's frames, and the event that says they are on the host
+    uint32_t *d_H = nullptr;
+    uint8_t *h_H = nullptr;
+    cudaEvent_t hashed = nullptr;
     // work in flight
     bool busy = false;
     uint8_t *user_out = nullptr;  // where h_out goes once `done` fires (nullptr: D2H went straight to the caller)
@@ -109,6 +113,9 @@ void free_slot(Slot &s) {
     if (s.d_D) cudaFree(s.d_D);
     if (s.h_IR) cudaFreeHost(s.h_IR);
     if (s.d_IR) cudaFree(s.d_IR);
+    if (s.d_H) cudaFree(s.d_H);
+    if (s.h_H) cudaFreeHost(s.h_H);
+    if (s.hashed) cudaEventDestroy(s.hashed);
     if (s.h_status) cudaFreeHost(s.h_status);
     if (s.d_status) cudaFree(s.d_status);
     if (s.done) cudaEventDestroy(s.done);
@@ -127,6 +134,11 @@ int ensure_slot(vcrypt_ctx *c, Slot &s, bool need_hF, bool need_hout) {
     const bool generic = !c->plan.tiled || (c->p.flags & VCRYPT_FLAG_FORCE_GENERIC);
     if (generic && !s.d_out) VC_CUDA(c, cudaMalloc(&s.d_out, fb));
     if (!s.d_D) VC_CUDA(c, cudaMalloc(&s.d_D, db));
+    if (c->p.flags & VCRYPT_FLAG_DEVICE_HASH) {
+        if (!s.d_H) VC_CUDA(c, cudaMalloc(&s.d_H, c->batch * 32u));
+        if (!s.h_H) VC_CUDA(c, cudaHostAlloc(&s.h_H, c->batch * 32u, cudaHostAllocDefault));
+        if (!s.hashed) VC_CUDA(c, cudaEventCreateWithFlags(&s.hashed, cudaEventDisableTiming));
+    }
     if (c->p.flags & VCRYPT_FLAG_DEVICE_DERIVE) {
         const size_t irb = c->batch * 2u * (size_t)c->p.n_workers * 4u * sizeof(double);
         if (!s.h_IR) VC_CUDA(c, cudaHostAlloc(&s.h_IR, irb, cudaHostAllocDefault));
@@ -248,7 +260,7 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
             } else {
                 c->cuda = true;
                 c->device = dev;
-                c->slots.resize(p->n_streams ? p->n_streams : 3);
+                c->slots.resize(p->n_streams ? p->n_streams : ((p->flags & VCRYPT_FLAG_DEVICE_HASH) ? 6 : 3));  // device hashing wants a deeper pipeline
             }
         }
     } catch (const std::bad_alloc &) {
@@ -413,6 +425,22 @@ extern "C" int vcrypt_derive(vcrypt_ctx *c, const uint8_t *hash, uint16_t *D_out
     return VCRYPT_OK;
 }
 
+extern "C" int vcrypt_frame_hash_device(vcrypt_ctx *c, const void *d_frames, size_t n, uint8_t *hashes_out, void *stream) {
+    if (!c || !d_frames || !hashes_out || n == 0) return VCRYPT_E_ARG;
+    if (!c->cuda) return VCRYPT_E_CUDA;
+    if ((((uintptr_t)d_frames) & 15u) || c->g.row_bytes % 16u != 0) return VCRYPT_E_SHAPE;
+    VC_CUDA(c, cudaSetDevice(c->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint32_t *d_H = nullptr;
+    cudaError_t e = cudaMalloc(&d_H, n * 32u);
+    if (e == cudaSuccess) e = vk::hash_device(c->g, static_cast<const uint8_t *>(d_frames), c->p.n_workers, n, d_H, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(hashes_out, d_H, n * 32u, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (d_H) cudaFree(d_H);
+    if (e != cudaSuccess) return cuda_fail(c, e, "device hashing");
+    return VCRYPT_OK;
+}
+
 extern "C" int vcrypt_derive_device(vcrypt_ctx *c, const uint8_t *hash, void *d_D, void *d_B, void *stream) {
     if (!c || !hash || !d_D || !d_B) return VCRYPT_E_ARG;
     if (!c->cuda) return VCRYPT_E_CUDA;
@@ -501,17 +529,27 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
     const bool in_pinned = is_pinned(in) && is_pinned(in + n * fb - 1);
     const bool out_pinned = is_pinned(out) && is_pinned(out + n * fb - 1);
     const bool generic = !c->plan.tiled || (c->p.flags & VCRYPT_FLAG_FORCE_GENERIC);
+    const bool dev_derive = (c->p.flags & VCRYPT_FLAG_DEVICE_DERIVE) != 0;
+    // device hashing needs 16-byte rows (128-bit loads); other shapes are hashed on the host: same bytes
+    const bool dev_hash = !decrypt && (c->p.flags & VCRYPT_FLAG_DEVICE_HASH) && c->g.row_bytes % 16u == 0;
+    const size_t S_ = c->slots.size();
+    const size_t nbatch = (n + c->batch - 1) / c->batch;
+    // Two stages per batch.  Stage A: staging, upload of the frames, hashing (host threads, or the GPU + an event).
+    // Stage B: chain + derivation, rest of the upload, cipher kernels, download.  With device hashing stage A runs
+    // S - 1 batches ahead, so that the host only waits for hashes that were requested long ago; otherwise A and B of a
+    // batch follow each other directly.
+    const size_t lag = dev_hash ? S_ - 1 : 0;
     double S[4];
     std::memcpy(S, c->S, sizeof S);
     int rc = VCRYPT_OK;
-    size_t k = 0;
-    for (size_t b0 = 0; b0 < n && rc == VCRYPT_OK; b0 += c->batch, ++k) {
-        const size_t m = n - b0 < c->batch ? n - b0 : c->batch;
-        Slot &s = c->slots[k % c->slots.size()];
-        if ((rc = retire_slot(c, s)) != VCRYPT_OK) break;
-        if ((rc = ensure_slot(c, s, !in_pinned, !out_pinned)) != VCRYPT_OK) break;
+
+    auto stage_a = [&](size_t k) -> int {
+        const size_t b0 = k * c->batch, m = n - b0 < c->batch ? n - b0 : c->batch;
+        Slot &s = c->slots[k % S_];
+        int r = retire_slot(c, s);
+        if (r != VCRYPT_OK) return r;
+        if ((r = ensure_slot(c, s, !in_pinned, !out_pinned)) != VCRYPT_OK) return r;
         const uint8_t *src = in + b0 * fb;
-        const uint8_t *hs = hashes_in ? hashes_in + 32u * b0 : nullptr;
         if (!in_pinned) {
             const auto t0 = clk::now();
             const size_t chunk = (size_t)1 << 20, total = m * fb, nch = (total + chunk - 1) / chunk;
@@ -523,25 +561,45 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
             c->stage_ms[2] += ms_since(t0);
         }
         // step 15, first part: the frames do not depend on the derivation, so their upload is enqueued first and runs
-        // while the host hashes and derives (it shortens the per-batch latency; the throughput is host-bound either way)
+        // while the host hashes and derives
         cudaError_t e = cudaMemcpyAsync(s.d_F, in_pinned ? src : s.h_F, m * fb, cudaMemcpyHostToDevice, s.st);
-        if (e != cudaSuccess) { rc = cuda_fail(c, e, "upload"); break; }
-        if (!decrypt) {  // Algorithm 1 steps 4-6
+        if (e != cudaSuccess) return cuda_fail(c, e, "upload");
+        if (dev_hash) {  // Algorithm 1 steps 4-6 on the GPU: one thread per (frame, band), H = xor of the band digests
+            e = vk::hash_device(c->g, s.d_F, c->p.n_workers, m, s.d_H, s.st);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(s.h_H, s.d_H, m * 32u, cudaMemcpyDeviceToHost, s.st);
+            if (e == cudaSuccess) e = cudaEventRecord(s.hashed, s.st);
+            if (e != cudaSuccess) return cuda_fail(c, e, "device hashing");
+            c->launches_last += 2;
+            c->launches_total += 2;
+        } else if (!decrypt) {  // Algorithm 1 steps 4-6 on the host threads
             const auto t0 = clk::now();
             hash_frames(c, src, m, hashes_out + 32u * b0);
-            hs = hashes_out + 32u * b0;
             c->stage_ms[0] += ms_since(t0);
         }
-        const bool dev_derive = (c->p.flags & VCRYPT_FLAG_DEVICE_DERIVE) != 0;
+        return VCRYPT_OK;
+    };
+
+    auto stage_b = [&](size_t k) -> int {
+        const size_t b0 = k * c->batch, m = n - b0 < c->batch ? n - b0 : c->batch;
+        Slot &s = c->slots[k % S_];
+        const uint8_t *hs = decrypt ? hashes_in + 32u * b0 : hashes_out + 32u * b0;
+        if (dev_hash) {
+            const auto t0 = clk::now();
+            const cudaError_t e = cudaEventSynchronize(s.hashed);
+            c->stage_ms[0] += ms_since(t0);
+            if (e != cudaSuccess) return cuda_fail(c, e, "device hashing");
+            std::memcpy(hashes_out + 32u * b0, s.h_H, m * 32u);
+        }
         {  // steps 7-14
             const auto t0 = clk::now();
-            rc = dev_derive ? chain_frames(c, S, hs, m, s.h_IR) : derive_frames(c, S, hs, m, s.h_D, s.h_B);
+            const int r = dev_derive ? chain_frames(c, S, hs, m, s.h_IR) : derive_frames(c, S, hs, m, s.h_D, s.h_B);
             c->stage_ms[1] += ms_since(t0);
-            if (rc != VCRYPT_OK) break;
+            if (r != VCRYPT_OK) return r;
         }
         // steps 15-21: rest of the upload, GPU steps, download -- asynchronous on the slot's stream
         uint8_t *d_res = generic ? s.d_out : s.d_F;
         uint8_t *h_res = out_pinned ? out + b0 * fb : s.h_out;
+        cudaError_t e;
         if (dev_derive) {  // the worker systems run on the GPU: only the LHCS_m records go up (2n x 32 bytes per frame)
             e = cudaMemcpyAsync(s.d_IR, s.h_IR, m * 2u * (size_t)c->p.n_workers * 4u * sizeof(double), cudaMemcpyHostToDevice, s.st);
             if (e == cudaSuccess) e = cudaMemsetAsync(s.d_status, 0, sizeof(uint32_t), s.st);
@@ -552,18 +610,25 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
             e = cudaMemcpyAsync(s.d_D, s.h_D, m * nD * sizeof(uint16_t), cudaMemcpyHostToDevice, s.st);
             if (e == cudaSuccess) e = cudaMemcpyAsync(s.d_B, s.h_B, m * fb, cudaMemcpyHostToDevice, s.st);
         }
-        if (e != cudaSuccess) { rc = cuda_fail(c, e, "upload"); break; }
-        if ((rc = launch_cipher(c, decrypt, s.d_F, s.d_D, s.d_B, m, d_res, s.st)) != VCRYPT_OK) break;
+        if (e != cudaSuccess) return cuda_fail(c, e, "upload");
+        const int r = launch_cipher(c, decrypt, s.d_F, s.d_D, s.d_B, m, d_res, s.st);
+        if (r != VCRYPT_OK) return r;
         e = cudaMemcpyAsync(h_res, d_res, m * fb, cudaMemcpyDeviceToHost, s.st);
         if (e == cudaSuccess) e = cudaEventRecord(s.done, s.st);
-        if (e != cudaSuccess) { rc = cuda_fail(c, e, "download"); break; }
+        if (e != cudaSuccess) return cuda_fail(c, e, "download");
         s.busy = true;
         s.user_out = out_pinned ? nullptr : out + b0 * fb;
         s.out_bytes = m * fb;
+        return VCRYPT_OK;
+    };
+
+    for (size_t k = 0; k < nbatch + lag && rc == VCRYPT_OK; ++k) {
+        if (k < nbatch) rc = stage_a(k);
+        if (rc == VCRYPT_OK && k >= lag) rc = stage_b(k - lag);
     }
     // drain in submission order
-    for (size_t i = 0; i < c->slots.size(); ++i) {
-        Slot &s = c->slots[(k + i) % c->slots.size()];
+    for (size_t i = 0; i < S_; ++i) {
+        Slot &s = c->slots[(nbatch + i) % S_];
         const int r2 = retire_slot(c, s);
         if (rc == VCRYPT_OK) rc = r2;
     }

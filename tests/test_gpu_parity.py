@@ -275,12 +275,41 @@ def test_device_derivation_matches_oracle(torch_cuda, vb, orc, w, h, n):
         assert np.array_equal(v.get_state()[0], vh.get_state()[0]) and v.get_state()[1] == vh.get_state()[1]
 
 
+@pytest.mark.parametrize("w,h,n,nf", [(64, 48, 32, 3), (64, 48, 1, 2), (16, 5, 8, 2), (80, 33, 7, 2), (256, 256, 32, 1), (640, 480, 6, 2),
+                                      (1920, 1080, 32, 2)])
+def test_device_hashing_matches_oracle(torch_cuda, vb, orc, w, h, n, nf):
+    """NEXT-2: H = xor of the band SHA-256 digests computed on the GPU equals the oracle's (and hashlib's for
+    n = 1), over bands of unequal height, empty bands (n > h), tails of 0 / 16 / 32 / 48 bytes."""
+    import hashlib
+
+    torch = torch_cuda
+    F = synth.random_frames(w, h, nf, seed=w + h + n)
+    v = gpu_ctx(vb, w, h, n=n)
+    Hs = v.frame_hash_device(torch.from_numpy(F).cuda())
+    for k in range(nf):
+        assert Hs[k].tobytes() == orc.frame_hash(F[k], n), k
+        assert Hs[k].tobytes() == v.frame_hash(F[k])
+        if n == 1:
+            assert Hs[k].tobytes() == hashlib.sha256(F[k].tobytes()).digest()
+
+
+def test_device_hashing_rejects_unaligned_rows(torch_cuda, vb):
+    torch = torch_cuda
+    v = gpu_ctx(vb, 17, 9, n=3)
+    F = torch.zeros((1, 9, 17, 3), dtype=torch.uint8, device="cuda")
+    out = np.empty((1, 32), np.uint8)
+    assert v.L.vcrypt_frame_hash_device(v._p, F.data_ptr(), 1, out.ctypes.data, 0) == vb.E_SHAPE
+
+
+@pytest.mark.parametrize("flags", ["derive", "hash", "both"])
 @pytest.mark.parametrize("cfgname,nframes", [("C1", 1), ("C2", 24), ("C4", 20)])
-def test_whole_path_with_device_derivation(vb, orc, cfgname, nframes):
-    """vcrypt_encrypt_frames / vcrypt_decrypt_frames with VCRYPT_FLAG_DEVICE_DERIVE: same ciphertext, hashes and plaintext."""
+def test_whole_path_with_device_derivation(vb, orc, cfgname, nframes, flags):
+    """vcrypt_encrypt_frames / vcrypt_decrypt_frames with VCRYPT_FLAG_DEVICE_DERIVE and / or VCRYPT_FLAG_DEVICE_HASH
+    (two-stage pipeline, hashing running ahead): same ciphertext, hashes and plaintext."""
     cfg = synth.CONFIGS[cfgname]
     frames = synth.video(cfg, nframes)
-    enc = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams, flags=vb.FLAG_DEVICE_DERIVE)
+    fl = {"derive": vb.FLAG_DEVICE_DERIVE, "hash": vb.FLAG_DEVICE_HASH, "both": vb.FLAG_DEVICE_DERIVE | vb.FLAG_DEVICE_HASH}[flags]
+    enc = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams if flags == "derive" else 0, flags=fl)
     C, Hs = enc.encrypt_frames(frames)
     ref = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
     C2, H2 = ref.encrypt_frames(frames)
@@ -289,7 +318,7 @@ def test_whole_path_with_device_derivation(vb, orc, cfgname, nframes):
     k = min(2, nframes)
     Co, Ho = oc.encrypt_frames(frames[:k])
     assert np.array_equal(C[:k], Co) and np.array_equal(Hs[:k], Ho)
-    dec = gpu_ctx(vb, cfg.w, cfg.h, batch=3, n_streams=2, flags=vb.FLAG_DEVICE_DERIVE)
+    dec = gpu_ctx(vb, cfg.w, cfg.h, batch=3, n_streams=2, flags=fl)
     assert np.array_equal(dec.decrypt_frames(C, Hs), frames)
     assert enc.get_state()[1] == nframes and np.array_equal(enc.get_state()[0], ref.get_state()[0])
 
