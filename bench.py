@@ -8,8 +8,9 @@ One "step" = one pass of the whole hot path over the clip of the chosen config (
   value : frames/s with F_o, D, B already resident in HBM -- vcrypt_encrypt_device calls only (rows a6-a10),
           timed with CUDA events on the launching stream.
   e2e   : frames/s through vcrypt_encrypt_frames with pinned HOST buffers: sub-frame SHA-256, chain, worker
-          LHCS -> D, B (on the GPU with --derive device, the default; on the host lanes with --derive host: same
-          bytes), H2D, kernels, D2H all inside the timed region (rows a1-a11), wall clock.
+          LHCS -> D, B, H2D, kernels, D2H all inside the timed region (rows a1-a11), wall clock.  By default the band
+          hashes and the worker systems run on the GPU (--hash device --derive device, pipeline 12 deep); --hash host
+          --derive host is the all-host derivation with the config's 3 streams: same bytes.
   roofline : algorithmic bytes (9wh per frame + D) / CUDA-event time of the encrypt kernels vs the measured HBM peak.
   cpu_baseline : the oracle as it stands on a bounded sample, one core.
 Prints ONE JSON line (rank 0).  Under torchrun (N > 1) every rank encrypts its own clip (weak scaling, no
@@ -131,7 +132,8 @@ def run_reference(args, cfg):
 
 def workload_name(cfg):
     return (f"{cfg.name}: {cfg.w}x{cfg.h}x3 uint8 synthetic video (moving gradient + blocks + noise), {cfg.frames} frames, "
-            f"batches of {cfg.batch} per call, {cfg.n_streams} streams, key = 4 doubles, n_workers = {synth.N_WORKERS}")
+            f"batches of {cfg.batch} per call, {cfg.n_streams} streams (all-host derivation; the e2e leg's actual depth is e2e.n_streams), "
+            f"key = 4 doubles, n_workers = {synth.N_WORKERS}")
 
 
 def main():
@@ -143,14 +145,20 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--frames", type=int, default=0, help="frames per step (default: the config's clip length)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--derive", default="device", choices=["host", "device"],
+    ap.add_argument("--derive", default="auto", choices=["auto", "host", "device"],
                     help="where the worker systems (D, B) of the end-to-end leg run: host lanes or the GPU (same bytes)")
-    ap.add_argument("--hash", default="host", choices=["host", "device"],
+    ap.add_argument("--hash", default="auto", choices=["auto", "host", "device"],
                     help="where the sub-frame SHA-256 of the end-to-end leg runs (same H)")
+    ap.add_argument("--hash-bands", type=int, default=0, help="with --hash device: row bands per frame hashed on the GPU (0: all)")
     ap.add_argument("--e2e-batch", type=int, default=0, help="frames per pipeline slot of the end-to-end leg (0: the config's)")
     ap.add_argument("--e2e-streams", type=int, default=0, help="pipeline depth of the end-to-end leg (0: the config's)")
     args = ap.parse_args()
     cfg = synth.CONFIGS[args.config]
+    # auto: throughput configs (batches of several frames) put band hashing and worker systems on the GPU; the one-frame-
+    # per-call latency config (C3) keeps them on the host threads (a GPU thread needs 6 ms per band, 2.6 ms per chain)
+    for k in ("derive", "hash"):
+        if getattr(args, k) == "auto":
+            setattr(args, k, "device" if (args.e2e_batch or cfg.batch) >= 4 else "host")
     if args.impl == "reference":
         return run_reference(args, cfg)
 
@@ -259,14 +267,18 @@ def main():
         for which, name in ((0, "sequential_copy"), (1, "two_pass_traffic_sequential"), (2, "column_strips_read_write")):
             probes[name] = kctx.memory_probe(which, nb, 20) / nb  # us per frame
 
+    # pipeline depth of the end-to-end leg: the config's 3 streams with host hashing; device hashing (6 ms per band on a
+    # GPU thread) needs a deeper pipeline to be hidden (results do not depend on it)
+    e2e_streams = args.e2e_streams or (12 if args.hash == "device" else cfg.n_streams)
     # ---- end to end through the host-buffer call -----------------------------------------------------------
     ectx = None
     e2e_s = []
     for k in range(W + K):
         ectx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=args.e2e_batch or cfg.batch,
-                         n_streams=args.e2e_streams or cfg.n_streams, host_threads=threads, device=local,
+                         n_streams=e2e_streams, host_threads=threads, device=local,
                          flags=(vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0) |
-                         (vb.FLAG_DEVICE_HASH if args.hash == "device" else 0)) if ectx is None else ectx
+                         (vb.FLAG_DEVICE_HASH if args.hash == "device" else 0),
+                         device_hash_bands=args.hash_bands) if ectx is None else ectx
         if k == W:
             barrier()
             t_e2e0 = time.perf_counter()
@@ -325,7 +337,7 @@ def main():
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": T * ((fb + 64 * synth.N_WORKERS) if args.derive == "device" else (2 * fb + 2 * nD)),
                 "d2h_bytes_per_step": T * fb,
                 "ms_per_frame": 1e3 * e2e_total / (K * T), "ms_per_step_median": 1e3 * statistics.median(e2e_s),
-                "stage_ms_last_call": stage, "derive": args.derive, "hash": args.hash, "batch": args.e2e_batch or cfg.batch, "n_streams": args.e2e_streams or cfg.n_streams,
+                "stage_ms_last_call": stage, "derive": args.derive, "hash": args.hash, "hash_bands_on_gpu": (args.hash_bands or synth.N_WORKERS) if args.hash == "device" else 0, "batch": args.e2e_batch or cfg.batch, "n_streams": e2e_streams,
                 "timer": "wall clock around vcrypt_encrypt_frames, pinned host in/out"},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

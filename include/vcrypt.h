@@ -61,7 +61,8 @@ extern "C" {
 #define VCRYPT_FLAG_DEVICE_DERIVE 8u  /* worker systems -> D, B on the GPU (same bytes): the host only
                                          hashes and runs the serial LHCS_m chain; D and B never cross PCIe */
 #define VCRYPT_FLAG_DEVICE_HASH 16u   /* sub-frame SHA-256 of vcrypt_encrypt_frames on the GPU, on the frames it
-                                         uploads anyway (same H); shapes with 3W % 16 != 0 are hashed on the host */
+                                         uploads anyway, shared with the host threads band by band (device_hash_bands;
+                                         same H); shapes with 3W % 16 != 0 are hashed on the host only */
 
 typedef struct vcrypt_ctx vcrypt_ctx; /* opaque: chain state, host thread pool, streams, device and pinned buffers */
 
@@ -72,10 +73,13 @@ typedef struct vcrypt_params {
                                NOT the number of host threads                                                      */
     uint32_t width, height; /* w, h; channels fixed at 3                                                          */
     uint32_t batch;         /* frames per kernel launch in the host-buffer pipeline (0 -> 8)                      */
-    uint32_t n_streams;     /* pipeline depth: streams / staging slots (0 -> 3)                                   */
+    uint32_t n_streams;     /* pipeline depth: streams / staging slots (0 -> 3; 12 with VCRYPT_FLAG_DEVICE_HASH)   */
     uint32_t host_threads;  /* host threads for hashing and derivation (0 -> hardware concurrency)                */
     uint32_t flags;         /* VCRYPT_FLAG_*                                                                      */
     int32_t device;         /* CUDA device ordinal (-1 -> current device)                                         */
+    uint32_t device_hash_bands; /* with VCRYPT_FLAG_DEVICE_HASH: how many of the n row bands of every frame the GPU
+                               hashes (the last ones; the host threads hash the others at the same time);
+                               0 or values above n -> all n.  Does not affect results                          */
 } vcrypt_params;
 
 /* Algorithm 1 set-up (PAPER.md:85 steps 1-2): validates the parameters, whitens the key (reading Q5 of

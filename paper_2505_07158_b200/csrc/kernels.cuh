@@ -61,9 +61,10 @@ cudaError_t decrypt_generic(const Geom &g, const uint8_t *src, const uint16_t *D
 cudaError_t derive_device(const Geom &g, const double *d_IR, double gamma, uint32_t n, size_t m, uint16_t *d_D, uint8_t *d_B,
                           uint32_t *d_status, cudaStream_t st);
 
-// Device-side sub-frame hashing (sha256.cu): H of m frames (n row bands each, xor of their SHA-256 digests) into d_H
-// (m x 32 bytes, digest byte order).  Needs 16-byte aligned frames and row_bytes % 16 == 0 (cudaErrorInvalidValue otherwise).
-cudaError_t hash_device(const Geom &g, const uint8_t *d_frames, uint32_t n, size_t m, uint32_t *d_H, cudaStream_t st);
+// Device-side sub-frame hashing (sha256.cu): xor of the SHA-256 digests of row bands band0 .. n-1 of each of m frames
+// into d_H (m x 32 bytes, digest byte order).  Needs 16-byte aligned frames and row_bytes % 16 == 0 (cudaErrorInvalidValue otherwise).
+cudaError_t hash_device(const Geom &g, const uint8_t *d_frames, uint32_t n, uint32_t band0, size_t m, uint32_t *d_H,
+                        cudaStream_t st);
 
 // Memory-system probes (membench.cu): see vcrypt_memory_probe in include/vcrypt.h.
 cudaError_t memory_probe(const Geom &g, int which, size_t frames, int reps, cudaStream_t st, double *us_per_call);

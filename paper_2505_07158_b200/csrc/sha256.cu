@@ -48,11 +48,12 @@ __device__ __forceinline__ void compress(uint32_t (&st)[8], uint32_t (&w)[16]) {
 }  // namespace
 
 // frames: m x (h x 3w) bytes, 16-byte aligned, row_bytes % 16 == 0.  H: m x 8 words, zeroed by the caller; on exit
-// H[f] holds the xor of the n band digests as big-endian words (byte-swapped to digest order by finish_hash_kernel).
-__global__ void __launch_bounds__(32) sha_bands_kernel(const uint8_t *__restrict__ frames, Geom g, uint32_t n, uint32_t m, uint32_t *H) {
-    const uint32_t t = blockIdx.x * 32u + threadIdx.x;
-    if (t >= m * n) return;
-    const uint32_t f = t / n, band = t - f * n;
+// H[f] holds the xor of the digests of bands band0 .. n-1 as big-endian words (byte-swapped to digest order by finish_hash_kernel).
+__global__ void __launch_bounds__(32) sha_bands_kernel(const uint8_t *__restrict__ frames, Geom g, uint32_t n, uint32_t band0,
+                                                       uint32_t m, uint32_t *H) {
+    const uint32_t t = blockIdx.x * 32u + threadIdx.x, nb = n - band0;  // bands band0 .. n-1 of every frame
+    if (t >= m * nb) return;
+    const uint32_t f = t / nb, band = band0 + (t - f * nb);
     const uint64_t r0 = ((uint64_t)band * g.h) / n, r1 = ((uint64_t)(band + 1u) * g.h) / n;
     const uint64_t len = (r1 - r0) * g.row_bytes;
     const uint8_t *msg = frames + (size_t)f * g.frame_bytes + r0 * g.row_bytes;
@@ -106,13 +107,14 @@ __global__ void finish_hash_kernel(uint32_t *H, uint32_t nwords) {
     if (i < nwords) H[i] = __byte_perm(H[i], 0u, 0x0123);
 }
 
-cudaError_t hash_device(const Geom &g, const uint8_t *d_frames, uint32_t n, size_t m, uint32_t *d_H, cudaStream_t st) {
-    if (!m) return cudaSuccess;
+cudaError_t hash_device(const Geom &g, const uint8_t *d_frames, uint32_t n, uint32_t band0, size_t m, uint32_t *d_H,
+                        cudaStream_t st) {
+    if (!m || band0 >= n) return m ? cudaMemsetAsync(d_H, 0, m * 32u, st) : cudaSuccess;
     if (g.row_bytes % 16u != 0u || (reinterpret_cast<uintptr_t>(d_frames) & 15u)) return cudaErrorInvalidValue;
     cudaError_t e = cudaMemsetAsync(d_H, 0, m * 32u, st);
     if (e != cudaSuccess) return e;
-    const uint32_t total = (uint32_t)(m * n);
-    sha_bands_kernel<<<(total + 31u) / 32u, 32, 0, st>>>(d_frames, g, n, (uint32_t)m, d_H);
+    const uint32_t total = (uint32_t)(m * (n - band0));
+    sha_bands_kernel<<<(total + 31u) / 32u, 32, 0, st>>>(d_frames, g, n, band0, (uint32_t)m, d_H);
     finish_hash_kernel<<<(unsigned)((m * 8u + 127u) / 128u), 128, 0, st>>>(d_H, (uint32_t)(m * 8u));
     return cudaGetLastError();
 }

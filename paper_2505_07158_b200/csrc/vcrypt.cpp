@@ -260,7 +260,7 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
             } else {
                 c->cuda = true;
                 c->device = dev;
-                c->slots.resize(p->n_streams ? p->n_streams : ((p->flags & VCRYPT_FLAG_DEVICE_HASH) ? 6 : 3));  // device hashing wants a deeper pipeline
+                c->slots.resize(p->n_streams ? p->n_streams : ((p->flags & VCRYPT_FLAG_DEVICE_HASH) ? 12 : 3));  // device hashing wants a deep pipeline (6 ms per band)
             }
         }
     } catch (const std::bad_alloc &) {
@@ -355,21 +355,22 @@ extern "C" int vcrypt_last_stage_ms(const vcrypt_ctx *c, double out[4]) {
 namespace {
 
 // H of m frames: every (frame, sub-frame) pair is one job; H = xor of the sub-frame digests.
-void hash_frames(vcrypt_ctx *c, const uint8_t *frames, size_t m, uint8_t *hashes) {
+// Only bands 0 .. nb-1 of every frame are hashed here (nb = n: the whole frame; fewer when the GPU takes the rest).
+void hash_frames(vcrypt_ctx *c, const uint8_t *frames, size_t m, uint8_t *hashes, uint32_t nb) {
     const uint32_t n = c->p.n_workers, h = c->g.h;
     const size_t rb = c->g.row_bytes, fb = c->g.frame_bytes;
     uint8_t *sub = c->subhash.data();
     const bool simd = c->simd;
-    c->pool->parallel_for(m * n, [&](size_t job) {
-        const size_t f = job / n;
-        const uint32_t k = (uint32_t)(job - f * n);
+    c->pool->parallel_for(m * nb, [&](size_t job) {
+        const size_t f = job / nb;
+        const uint32_t k = (uint32_t)(job - f * nb);
         const size_t r0 = vh::band_row(k, n, h), r1 = vh::band_row(k + 1, n, h);
-        vh::sha256(frames + f * fb + r0 * rb, (r1 - r0) * rb, sub + job * 32u, simd);
+        vh::sha256(frames + f * fb + r0 * rb, (r1 - r0) * rb, sub + (f * n + k) * 32u, simd);
     });
     for (size_t f = 0; f < m; ++f) {
         uint8_t *H = hashes + 32u * f;
         std::memset(H, 0, 32);
-        for (uint32_t k = 0; k < n; ++k)
+        for (uint32_t k = 0; k < nb; ++k)
             for (int b = 0; b < 32; ++b) H[b] ^= sub[(f * n + k) * 32u + b];
     }
 }
@@ -410,7 +411,7 @@ int chain_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, do
 
 extern "C" int vcrypt_frame_hash(vcrypt_ctx *c, const uint8_t *frame, uint8_t *H_out) {
     if (!c || !frame || !H_out) return VCRYPT_E_ARG;
-    hash_frames(c, frame, 1, H_out);
+    hash_frames(c, frame, 1, H_out, c->p.n_workers);
     return VCRYPT_OK;
 }
 
@@ -433,7 +434,7 @@ extern "C" int vcrypt_frame_hash_device(vcrypt_ctx *c, const void *d_frames, siz
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     uint32_t *d_H = nullptr;
     cudaError_t e = cudaMalloc(&d_H, n * 32u);
-    if (e == cudaSuccess) e = vk::hash_device(c->g, static_cast<const uint8_t *>(d_frames), c->p.n_workers, n, d_H, st);
+    if (e == cudaSuccess) e = vk::hash_device(c->g, static_cast<const uint8_t *>(d_frames), c->p.n_workers, 0, n, d_H, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(hashes_out, d_H, n * 32u, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (d_H) cudaFree(d_H);
@@ -532,13 +533,17 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
     const bool dev_derive = (c->p.flags & VCRYPT_FLAG_DEVICE_DERIVE) != 0;
     // device hashing needs 16-byte rows (128-bit loads); other shapes are hashed on the host: same bytes
     const bool dev_hash = !decrypt && (c->p.flags & VCRYPT_FLAG_DEVICE_HASH) && c->g.row_bytes % 16u == 0;
+    // the GPU hashes the last `dev_bands` row bands of every frame, the host threads the others at the same time
+    const uint32_t nw = c->p.n_workers;
+    const uint32_t dev_bands = !dev_hash ? 0u : c->p.device_hash_bands == 0 || c->p.device_hash_bands > nw ? nw : c->p.device_hash_bands;
+    const uint32_t host_bands = nw - dev_bands;
     const size_t S_ = c->slots.size();
     const size_t nbatch = (n + c->batch - 1) / c->batch;
     // Two stages per batch.  Stage A: staging, upload of the frames, hashing (host threads, or the GPU + an event).
     // Stage B: chain + derivation, rest of the upload, cipher kernels, download.  With device hashing stage A runs
-    // S - 1 batches ahead, so that the host only waits for hashes that were requested long ago; otherwise A and B of a
-    // batch follow each other directly.
-    const size_t lag = dev_hash ? S_ - 1 : 0;
+    // S / 2 batches ahead, so that the host only waits for hashes that were requested long ago and a slot's stage B has
+    // S / 2 iterations to finish before the slot is reused; otherwise A and B of a batch follow each other directly.
+    const size_t lag = dev_hash ? S_ / 2 : 0;
     double S[4];
     std::memcpy(S, c->S, sizeof S);
     int rc = VCRYPT_OK;
@@ -564,16 +569,17 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
         // while the host hashes and derives
         cudaError_t e = cudaMemcpyAsync(s.d_F, in_pinned ? src : s.h_F, m * fb, cudaMemcpyHostToDevice, s.st);
         if (e != cudaSuccess) return cuda_fail(c, e, "upload");
-        if (dev_hash) {  // Algorithm 1 steps 4-6 on the GPU: one thread per (frame, band), H = xor of the band digests
-            e = vk::hash_device(c->g, s.d_F, c->p.n_workers, m, s.d_H, s.st);
+        if (dev_hash) {  // Algorithm 1 steps 4-6, the GPU's share: one thread per (frame, band), xor of the band digests
+            e = vk::hash_device(c->g, s.d_F, nw, host_bands, m, s.d_H, s.st);
             if (e == cudaSuccess) e = cudaMemcpyAsync(s.h_H, s.d_H, m * 32u, cudaMemcpyDeviceToHost, s.st);
             if (e == cudaSuccess) e = cudaEventRecord(s.hashed, s.st);
             if (e != cudaSuccess) return cuda_fail(c, e, "device hashing");
             c->launches_last += 2;
             c->launches_total += 2;
-        } else if (!decrypt) {  // Algorithm 1 steps 4-6 on the host threads
+        }
+        if (!decrypt) {  // Algorithm 1 steps 4-6 on the host threads (all bands, or the host's share)
             const auto t0 = clk::now();
-            hash_frames(c, src, m, hashes_out + 32u * b0);
+            hash_frames(c, src, m, hashes_out + 32u * b0, host_bands);
             c->stage_ms[0] += ms_since(t0);
         }
         return VCRYPT_OK;
@@ -588,7 +594,7 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
             const cudaError_t e = cudaEventSynchronize(s.hashed);
             c->stage_ms[0] += ms_since(t0);
             if (e != cudaSuccess) return cuda_fail(c, e, "device hashing");
-            std::memcpy(hashes_out + 32u * b0, s.h_H, m * 32u);
+            for (size_t i = 0; i < m * 32u; ++i) hashes_out[32u * b0 + i] ^= s.h_H[i];  // host share xor device share
         }
         {  // steps 7-14
             const auto t0 = clk::now();
