@@ -166,6 +166,36 @@ int vcrypt_frame_hash_device(vcrypt_ctx *ctx, const void *d_frames, size_t n, ui
  * Advances the chain by one frame on success. */
 int vcrypt_derive_device(vcrypt_ctx *ctx, const uint8_t *hash, void *d_D, void *d_B, void *cuda_stream);
 
+/* ---- statistical evaluation of frames resident in device memory (PAPER.md sections III-IV) ---------------- */
+
+/* Per frame and channel c = 0..2 (index of the HWC buffer). */
+typedef struct vcrypt_frame_stats {
+    double hist_variance[3]; /* Eq. 4: (1/256^2) sum_i sum_j (z_i - z_j)^2 / 2 of the 256-bin histogram   */
+    double chi2[3];          /* Eq. 5 (:177): sum_i (z_i - N/256)^2 / (N/256), N = W*H                                    */
+    double entropy[3];       /* Eq. 10 (:345): sum_i p_i log2(1/p_i), bits                                                */
+    double corr[3][3];       /* Eq. 6-9 (:283-294): correlation coefficient of ALL adjacent pairs, [channel][direction]:
+                                0 horizontal (i,j)-(i,j+1), 1 vertical (i,j)-(i+1,j), 2 diagonal (i,j)-(i+1,j+1);
+                                NaN when a variance is zero or there is no pair                                          */
+} vcrypt_frame_stats;
+
+/* Histogram variance, chi^2, entropy and adjacent-pixel correlation of n frames (one pass over each frame on the GPU;
+ * exact integer sums on the device, the final floating-point steps on the host in binary64).
+ * d_frames: device, n x H x W x 3.  stats_out: host, n entries.  hist_out: host, n x 3 x 256 uint32, or NULL. */
+int vcrypt_frame_stats_device(vcrypt_ctx *ctx, const void *d_frames, size_t n, vcrypt_frame_stats *stats_out,
+                              uint32_t *hist_out, void *cuda_stream);
+
+/* NPCR (Eq. 14, 16) and UACI (Eq. 15) in percent between frames d_a[k] and d_b[k], k < n:
+ * npcr_out, uaci_out: host, n x 4 doubles = {all three channels together, channel 0, 1, 2}. */
+int vcrypt_npcr_uaci_device(vcrypt_ctx *ctx, const void *d_a, const void *d_b, size_t n, double *npcr_out, double *uaci_out,
+                            void *cuda_stream);
+
+/* Local Shannon entropy (Eq. 11): mean over k square blocks (side x side pixels, top-left pixel
+ * (x, y) = blocks_xy[2b], blocks_xy[2b+1], chosen by the caller: non-overlapping, inside the frame) of the entropy of
+ * each block's histogram, per channel.  The paper's setting is k = 30, side = 44 (T_B = 1936).
+ * out: host, n x 3 doubles.  VCRYPT_E_ARG if a block leaves the frame. */
+int vcrypt_local_entropy_device(vcrypt_ctx *ctx, const void *d_frames, size_t n, const uint32_t *blocks_xy, uint32_t k,
+                                uint32_t side, double *out, void *cuda_stream);
+
 /* Memory-system probe (bench hook): moves the bytes of one vcrypt_encrypt_device call on `frames` frames of this
  * context's shape with no cipher arithmetic, `reps` times on the context's device, and returns the mean time of
  * one repetition in microseconds (CUDA events).  which = 0: sequential copy (read 3wh + write 3wh per frame);

@@ -24,6 +24,11 @@ class Params(C.Structure):
                 ("flags", C.c_uint32), ("device", C.c_int32), ("device_hash_bands", C.c_uint32)]
 
 
+class FrameStats(C.Structure):
+    _fields_ = [("hist_variance", C.c_double * 3), ("chi2", C.c_double * 3), ("entropy", C.c_double * 3),
+                ("corr", (C.c_double * 3) * 3)]
+
+
 class VcryptError(RuntimeError):
     def __init__(self, code: int, what: str, detail: str = ""):
         self.code = code
@@ -67,6 +72,9 @@ def lib() -> C.CDLL:
     L.vcrypt_last_stage_ms.argtypes = [_vp, C.POINTER(C.c_double)]
     L.vcrypt_derive_device.argtypes = [_vp, _vp, _vp, _vp, _vp]
     L.vcrypt_frame_hash_device.argtypes = [_vp, _vp, C.c_size_t, _vp, _vp]
+    L.vcrypt_frame_stats_device.argtypes = [_vp, _vp, C.c_size_t, C.POINTER(FrameStats), _vp, _vp]
+    L.vcrypt_npcr_uaci_device.argtypes = [_vp, _vp, _vp, C.c_size_t, _vp, _vp, _vp]
+    L.vcrypt_local_entropy_device.argtypes = [_vp, _vp, C.c_size_t, _vp, C.c_uint32, C.c_uint32, _vp, _vp]
     L.vcrypt_memory_probe.argtypes = [_vp, C.c_int, C.c_size_t, C.c_int, C.POINTER(C.c_double)]
     _lib = L
     return L
@@ -232,6 +240,36 @@ class Vcrypt:
         a, b = C.c_uint64(), C.c_uint64()
         self._check(self.L.vcrypt_launch_count(self._p, C.byref(a), C.byref(b)), "vcrypt_launch_count")
         return int(a.value), int(b.value)
+
+    def frame_stats_device(self, d_frames, stream=None):
+        """vcrypt_frame_stats_device -> dict of arrays: hist_variance, chi2, entropy (n, 3), corr (n, 3, 3), hist (n, 3, 256)."""
+        n = int(d_frames.shape[0])
+        st = (FrameStats * n)()
+        hist = np.empty((n, 3, 256), np.uint32)
+        self._check(self.L.vcrypt_frame_stats_device(self._p, _dev_ptr(d_frames, n * self.frame_bytes, "d_frames"), n, st,
+                                                     hist.ctypes.data, 0 if stream is None else int(stream)), "vcrypt_frame_stats_device")
+        return {"hist_variance": np.array([list(x.hist_variance) for x in st]), "chi2": np.array([list(x.chi2) for x in st]),
+                "entropy": np.array([list(x.entropy) for x in st]),
+                "corr": np.array([[list(row) for row in x.corr] for x in st]), "hist": hist}
+
+    def npcr_uaci_device(self, d_a, d_b, stream=None):
+        """vcrypt_npcr_uaci_device -> (npcr, uaci), each (n, 4): all channels, channel 0, 1, 2 (percent)."""
+        n = int(d_a.shape[0])
+        npcr, uaci = np.empty((n, 4)), np.empty((n, 4))
+        self._check(self.L.vcrypt_npcr_uaci_device(self._p, _dev_ptr(d_a, n * self.frame_bytes, "d_a"),
+                                                   _dev_ptr(d_b, n * self.frame_bytes, "d_b"), n, npcr.ctypes.data, uaci.ctypes.data,
+                                                   0 if stream is None else int(stream)), "vcrypt_npcr_uaci_device")
+        return npcr, uaci
+
+    def local_entropy_device(self, d_frames, blocks_xy, side: int, stream=None):
+        """vcrypt_local_entropy_device -> (n, 3): mean block entropy per channel; blocks_xy (k, 2) uint32 top-left (x, y)."""
+        n = int(d_frames.shape[0])
+        xy = np.ascontiguousarray(blocks_xy, dtype=np.uint32)
+        out = np.empty((n, 3))
+        self._check(self.L.vcrypt_local_entropy_device(self._p, _dev_ptr(d_frames, n * self.frame_bytes, "d_frames"), n, xy.ctypes.data,
+                                                       xy.shape[0], side, out.ctypes.data, 0 if stream is None else int(stream)),
+                    "vcrypt_local_entropy_device")
+        return out
 
     def memory_probe(self, which: int, frames: int, reps: int = 20) -> float:
         """vcrypt_memory_probe: microseconds per repetition (0 sequential copy, 1 two-pass traffic, 2 column strips)."""

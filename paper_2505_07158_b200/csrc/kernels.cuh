@@ -66,6 +66,17 @@ cudaError_t derive_device(const Geom &g, const double *d_IR, double gamma, uint3
 cudaError_t hash_device(const Geom &g, const uint8_t *d_frames, uint32_t n, uint32_t band0, size_t m, uint32_t *d_H,
                         cudaStream_t st);
 
+// Statistical evaluation (stats.cu): exact integer sufficient statistics of frames in device memory.
+//   stats_device     : d_hist n x 3 x 256 u32 (per channel histogram), d_pairs n x 3 x 3 x 5 u64 (per channel and direction
+//                      H, V, D: sum x, sum y, sum xy, sum x^2, sum y^2 over all adjacent pairs)
+//   diff_device      : d_out n x 3 x 2 u64 (per channel: differing bytes, sum |a - b|)
+//   block_hist_device: d_bh n x k x 3 x 256 u32 (per block and channel histogram; d_xy k x 2 top-left corners, device)
+cudaError_t stats_device(const Geom &g, const uint8_t *d_frames, size_t n, uint32_t *d_hist, unsigned long long *d_pairs,
+                         cudaStream_t st);
+cudaError_t diff_device(const Geom &g, const uint8_t *d_a, const uint8_t *d_b, size_t n, unsigned long long *d_out, cudaStream_t st);
+cudaError_t block_hist_device(const Geom &g, const uint8_t *d_frames, size_t n, const uint32_t *d_xy, uint32_t k, uint32_t side,
+                              uint32_t *d_bh, cudaStream_t st);
+
 // Memory-system probes (membench.cu): see vcrypt_memory_probe in include/vcrypt.h.
 cudaError_t memory_probe(const Geom &g, int which, size_t frames, int reps, cudaStream_t st, double *us_per_call);
 

@@ -504,6 +504,135 @@ extern "C" int vcrypt_decrypt_device(vcrypt_ctx *c, const void *d_cipher, const 
     return device_call(c, true, d_cipher, d_D, d_B, n, d_plain, stream);
 }
 
+// =====================================================================================================
+// statistical evaluation (PAPER.md sections III-IV): exact integer sums from the GPU, final steps in binary64
+// =====================================================================================================
+namespace {
+
+double entropy_bits(const uint32_t *z, double total) {  // Eq. 10
+    double H = 0.0;
+    for (int i = 0; i < 256; ++i)
+        if (z[i]) {
+            const double p = (double)z[i] / total;
+            H += p * std::log2(1.0 / p);
+        }
+    return H;
+}
+
+}  // namespace
+
+extern "C" int vcrypt_frame_stats_device(vcrypt_ctx *c, const void *d_frames, size_t n, vcrypt_frame_stats *out, uint32_t *hist_out,
+                                         void *stream) {
+    if (!c || !d_frames || !out || n == 0) return VCRYPT_E_ARG;
+    if (!c->cuda) return VCRYPT_E_CUDA;
+    VC_CUDA(c, cudaSetDevice(c->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint32_t *d_hist = nullptr;
+    unsigned long long *d_pairs = nullptr;
+    std::vector<uint32_t> hist(n * 768u);
+    std::vector<unsigned long long> pairs(n * 45u);
+    cudaError_t e = cudaMalloc(&d_hist, n * 768u * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&d_pairs, n * 45u * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = vk::stats_device(c->g, static_cast<const uint8_t *>(d_frames), n, d_hist, d_pairs, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(hist.data(), d_hist, hist.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pairs.data(), d_pairs, pairs.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (d_hist) cudaFree(d_hist);
+    if (d_pairs) cudaFree(d_pairs);
+    if (e != cudaSuccess) return cuda_fail(c, e, "frame statistics");
+    const double N = (double)c->g.w * (double)c->g.h;
+    const uint64_t w = c->g.w, h = c->g.h;
+    const double npairs[3] = {(double)((w - 1) * h), (double)(w * (h - 1)), (double)((w - 1) * (h - 1))};
+    for (size_t f = 0; f < n; ++f) {
+        vcrypt_frame_stats &o = out[f];
+        for (int ch = 0; ch < 3; ++ch) {
+            const uint32_t *z = hist.data() + f * 768u + ch * 256u;
+            double s1 = 0.0, s2 = 0.0, chi = 0.0;
+            const double ex = N / 256.0;
+            for (int i = 0; i < 256; ++i) {
+                s1 += (double)z[i];
+                s2 += (double)z[i] * (double)z[i];
+                chi += ((double)z[i] - ex) * ((double)z[i] - ex) / ex;
+            }
+            // Eq. 4: (1/256^2) sum_i sum_j (z_i - z_j)^2 / 2 = (256 sum z^2 - (sum z)^2) / 256^2
+            o.hist_variance[ch] = (256.0 * s2 - s1 * s1) / 65536.0;
+            o.chi2[ch] = chi;
+            o.entropy[ch] = entropy_bits(z, N);
+            for (int d = 0; d < 3; ++d) {
+                const unsigned long long *p = pairs.data() + f * 45u + (ch * 3 + d) * 5;
+                const double M = npairs[d];
+                if (M <= 0.0) { o.corr[ch][d] = std::nan(""); continue; }
+                // Eq. 6-9 from the exact sums: cov = E[xy] - E[x]E[y], D(x) = E[x^2] - E[x]^2 (integer numerators)
+                const long double sx = (long double)p[0], sy = (long double)p[1], sxy = (long double)p[2], sxx = (long double)p[3],
+                                  syy = (long double)p[4], m = (long double)M;
+                const long double cov = m * sxy - sx * sy, dx = m * sxx - sx * sx, dy = m * syy - sy * sy;
+                o.corr[ch][d] = (dx > 0 && dy > 0) ? (double)(cov / std::sqrt(dx * dy)) : std::nan("");
+            }
+        }
+    }
+    if (hist_out) std::memcpy(hist_out, hist.data(), hist.size() * sizeof(uint32_t));
+    return VCRYPT_OK;
+}
+
+extern "C" int vcrypt_npcr_uaci_device(vcrypt_ctx *c, const void *d_a, const void *d_b, size_t n, double *npcr, double *uaci,
+                                       void *stream) {
+    if (!c || !d_a || !d_b || !npcr || !uaci || n == 0) return VCRYPT_E_ARG;
+    if (!c->cuda) return VCRYPT_E_CUDA;
+    VC_CUDA(c, cudaSetDevice(c->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned long long *d_out = nullptr;
+    std::vector<unsigned long long> r(n * 6u);
+    cudaError_t e = cudaMalloc(&d_out, r.size() * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = vk::diff_device(c->g, static_cast<const uint8_t *>(d_a), static_cast<const uint8_t *>(d_b), n, d_out, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(r.data(), d_out, r.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (d_out) cudaFree(d_out);
+    if (e != cudaSuccess) return cuda_fail(c, e, "NPCR / UACI");
+    const double N = (double)c->g.w * (double)c->g.h;
+    for (size_t f = 0; f < n; ++f) {
+        unsigned long long ne = 0, ad = 0;
+        for (int ch = 0; ch < 3; ++ch) {
+            const unsigned long long a = r[f * 6u + 2 * ch], b = r[f * 6u + 2 * ch + 1];
+            ne += a;
+            ad += b;
+            npcr[4 * f + 1 + ch] = 100.0 * (double)a / N;            // Eq. 14, 16
+            uaci[4 * f + 1 + ch] = 100.0 * (double)b / (N * 255.0);  // Eq. 15
+        }
+        npcr[4 * f] = 100.0 * (double)ne / (3.0 * N);
+        uaci[4 * f] = 100.0 * (double)ad / (3.0 * N * 255.0);
+    }
+    return VCRYPT_OK;
+}
+
+extern "C" int vcrypt_local_entropy_device(vcrypt_ctx *c, const void *d_frames, size_t n, const uint32_t *xy, uint32_t k, uint32_t side,
+                                           double *out, void *stream) {
+    if (!c || !d_frames || !xy || !out || n == 0 || k == 0 || side == 0) return VCRYPT_E_ARG;
+    if (!c->cuda) return VCRYPT_E_CUDA;
+    for (uint32_t b = 0; b < k; ++b)
+        if ((uint64_t)xy[2 * b] + side > c->g.w || (uint64_t)xy[2 * b + 1] + side > c->g.h) return VCRYPT_E_ARG;
+    VC_CUDA(c, cudaSetDevice(c->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint32_t *d_xy = nullptr, *d_bh = nullptr;
+    std::vector<uint32_t> bh(n * k * 768u);
+    cudaError_t e = cudaMalloc(&d_xy, 2u * k * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&d_bh, bh.size() * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_xy, xy, 2u * k * sizeof(uint32_t), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = vk::block_hist_device(c->g, static_cast<const uint8_t *>(d_frames), n, d_xy, k, side, d_bh, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(bh.data(), d_bh, bh.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (d_xy) cudaFree(d_xy);
+    if (d_bh) cudaFree(d_bh);
+    if (e != cudaSuccess) return cuda_fail(c, e, "local entropy");
+    const double TB = (double)side * (double)side;
+    for (size_t f = 0; f < n; ++f)
+        for (int ch = 0; ch < 3; ++ch) {
+            double acc = 0.0;
+            for (uint32_t b = 0; b < k; ++b) acc += entropy_bits(bh.data() + ((f * k + b) * 3u + ch) * 256u, TB);
+            out[3 * f + ch] = acc / (double)k;  // Eq. 11
+        }
+    return VCRYPT_OK;
+}
+
 extern "C" int vcrypt_memory_probe(vcrypt_ctx *c, int which, size_t frames, int reps, double *us_per_rep) {
     if (!c || !us_per_rep || which < 0 || which > 2 || frames == 0 || reps < 1) return VCRYPT_E_ARG;
     if (!c->cuda) return VCRYPT_E_CUDA;

@@ -105,6 +105,22 @@ def one_bit_pairs(cfg: Config | str, pairs: int, seed: int = 1003):
         yield f, g, (i, j, c, bit)
 
 
+def random_blocks(w: int, h: int, k: int, side: int, seed: int) -> np.ndarray:
+    """k non-overlapping side x side blocks inside a w x h frame (top-left (x, y), uint32), for the local Shannon entropy
+    test ("randomly selected, non-overlapping sub-blocks"); rejection sampling on a seeded generator."""
+    rng = np.random.default_rng(seed)
+    out = []
+    tries = 0
+    while len(out) < k:
+        tries += 1
+        if tries > 100000:
+            raise ValueError("cannot place the blocks")
+        x, y = int(rng.integers(0, w - side + 1)), int(rng.integers(0, h - side + 1))
+        if all(abs(x - a) >= side or abs(y - b) >= side for a, b in out):
+            out.append((x, y))
+    return np.array(out, dtype=np.uint32)
+
+
 def random_frames(w: int, h: int, frames: int, seed: int) -> np.ndarray:
     """i.i.d. uniform bytes, for odd shapes and edge cases."""
     return np.random.default_rng(seed).integers(0, 256, (frames, h, w, 3), dtype=np.uint8)
