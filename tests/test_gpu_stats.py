@@ -40,7 +40,9 @@ def frames_for(kind, w, h, nf, seed):
 
 
 @pytest.mark.parametrize("kind", ["random", "smooth"])
-@pytest.mark.parametrize("w,h,nf", [(64, 48, 2), (17, 9, 3), (1, 7, 1), (5, 1, 2), (130, 33, 1), (640, 480, 2)])
+# w % 4 == 0: DP4A fast path (incl. a single item per row, a single row, a single column of items); others: byte path
+@pytest.mark.parametrize("w,h,nf", [(64, 48, 2), (4, 6, 2), (8, 1, 2), (4, 1, 1), (132, 33, 1), (640, 480, 2), (1920, 1080, 1),
+                                    (17, 9, 3), (1, 7, 1), (5, 1, 2), (130, 33, 1)])
 def test_frame_stats_match_oracle(torch_cuda, vb, kind, w, h, nf):
     F = frames_for(kind, w, h, nf, seed=w * 7 + h)
     v = vb.Vcrypt(synth.KEY, synth.GAMMA, 4, w, h)
