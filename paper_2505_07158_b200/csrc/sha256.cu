@@ -1,11 +1,10 @@
 // sha256.cu -- device-side sub-frame hashing: h_m = SHA-256(f_m) for the n row bands of each
 // frame of a batch and H = xor_m h_m, on the frames that were uploaded for the cipher kernels anyway.
 //
-// SHA-256 (FIPS 180-4) is serial inside a message, so the parallelism is one thread per (frame, band): n x batch
-// independent message streams (256 at n = 32, batch = 8), one warp per CTA so that the warps spread over as many SMs as
-// possible.  A thread walks its band 64 bytes at a time with 128-bit loads, the next block in flight while the current
-// one is compressed (64 fully unrolled rounds on a 16-word rolling schedule), pads the tail as the standard says and
-// xors its digest into the frame's H with eight atomicXor.
+// SHA-256 (FIPS 180-4) is serial inside a message, so the parallelism is one message per (frame, band): n x batch
+// independent message streams (256 at n = 32, batch = 8), 32 messages per CTA so that the CTAs spread over as many SMs as
+// possible.  A band is walked 64 bytes at a time with 128-bit loads, the next block in flight while the current one is
+// processed, the tail padded as the standard says, and the digest xor-ed into the frame's H with eight atomicXor.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -28,78 +27,119 @@ __constant__ uint32_t KT[64] = {
 
 __device__ __forceinline__ uint32_t ror(uint32_t x, int n) { return __funnelshift_r(x, x, n); }
 __device__ __forceinline__ uint32_t bswap(uint32_t x) { return __byte_perm(x, 0u, 0x0123); }
-
-// One 64-byte block: w[] holds the 16 big-endian message words on entry (destroyed).
-__device__ __forceinline__ void compress(uint32_t (&st)[8], uint32_t (&w)[16]) {
-    uint32_t a = st[0], b = st[1], c = st[2], d = st[3], e = st[4], f = st[5], g = st[6], h = st[7];
-#pragma unroll
-    for (int t = 0; t < 64; ++t) {
-        if (t >= 16) {
-            const uint32_t w15 = w[(t + 1) & 15], w2 = w[(t + 14) & 15];
-            w[t & 15] += (ror(w15, 7) ^ ror(w15, 18) ^ (w15 >> 3)) + w[(t + 9) & 15] + (ror(w2, 17) ^ ror(w2, 19) ^ (w2 >> 10));
-        }
-        const uint32_t t1 = h + (ror(e, 6) ^ ror(e, 11) ^ ror(e, 25)) + (g ^ (e & (f ^ g))) + KT[t] + w[t & 15];
-        const uint32_t t2 = (ror(a, 2) ^ ror(a, 13) ^ ror(a, 22)) + ((a & b) | (c & (a | b)));
-        h = g; g = f; f = e; e = d + t1; d = c; c = b; b = a; a = t1 + t2;
-    }
-    st[0] += a; st[1] += b; st[2] += c; st[3] += d; st[4] += e; st[5] += f; st[6] += g; st[7] += h;
-}
+__device__ __forceinline__ void bar_sync(uint32_t id, uint32_t n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive(uint32_t id, uint32_t n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 }  // namespace
 
+// SHA-256 is serial inside a message, and a lone warp is bound by its own instruction stream (about 1 500 instructions per
+// 64-byte block, 2 cycles each on the ALU pipe).  The message schedule W_t (FIPS 180-4 section 6.2.2 step 1) does not
+// depend on the hash state, so a CTA is two warps working on the same 32 messages: the SCHEDULE warp loads the block,
+// expands W_0..63, adds K_t and leaves the 64 words in shared memory (double-buffered); the ROUND warp runs the 64 rounds
+// (step 3) reading them back.  The round warp is the longer of the two (about 960 instructions per block), the schedule warp
+// (about 650) runs one block ahead.  Hand-over with named barriers: FULL[buf] schedule -> round, EMPTY[buf] round -> schedule.
+//
 // frames: m x (h x 3w) bytes, 16-byte aligned, row_bytes % 16 == 0.  H: m x 8 words, zeroed by the caller; on exit
 // H[f] holds the xor of the digests of bands band0 .. n-1 as big-endian words (byte-swapped to digest order by finish_hash_kernel).
-__global__ void __launch_bounds__(32) sha_bands_kernel(const uint8_t *__restrict__ frames, Geom g, uint32_t n, uint32_t band0,
+__global__ void __launch_bounds__(64) sha_bands_kernel(const uint8_t *__restrict__ frames, Geom g, uint32_t n, uint32_t band0,
                                                        uint32_t m, uint32_t *H) {
-    const uint32_t t = blockIdx.x * 32u + threadIdx.x, nb = n - band0;  // bands band0 .. n-1 of every frame
-    if (t >= m * nb) return;
+    __shared__ uint32_t Wb[2][64][32];  // [buffer][t][lane]: W_t + K_t of the lane's current block
+    const uint32_t lane = threadIdx.x & 31u, role = threadIdx.x >> 5;  // role 0: rounds, 1: schedule
+    const uint32_t nb = n - band0, total = m * nb;                    // bands band0 .. n-1 of every frame
+    uint32_t t = blockIdx.x * 32u + lane;
+    const bool live = t < total;
+    if (!live) t = total - 1u;  // keeps both warps' loop bounds equal; a dead lane repeats the last message and writes nothing
     const uint32_t f = t / nb, band = band0 + (t - f * nb);
     const uint64_t r0 = ((uint64_t)band * g.h) / n, r1 = ((uint64_t)(band + 1u) * g.h) / n;
     const uint64_t len = (r1 - r0) * g.row_bytes;
-    const uint8_t *msg = frames + (size_t)f * g.frame_bytes + r0 * g.row_bytes;
-    const uint4 *p = reinterpret_cast<const uint4 *>(msg);
-    uint32_t st[8] = {0x6a09e667u, 0xbb67ae85u, 0x3c6ef372u, 0xa54ff53au, 0x510e527fu, 0x9b05688cu, 0x1f83d9abu, 0x5be0cd19u};
-    const uint64_t nblk = len >> 6;
-    uint4 nx[4];
-    if (nblk) {
+    const uint4 *p = reinterpret_cast<const uint4 *>(frames + (size_t)f * g.frame_bytes + r0 * g.row_bytes);
+    const uint32_t nblk = (uint32_t)(len >> 6);                      // whole blocks; one more block holds the tail and the padding
+    const uint32_t iters = __reduce_max_sync(0xffffffffu, nblk + 1u);  // the same in both warps: lane l holds the same message
+    constexpr uint32_t FULL = 1, EMPTY = 3;                           // named barriers FULL + buf, EMPTY + buf (64 threads each)
+
+    if (role == 1u) {
+        // ---------------- schedule warp ----------------
+        uint4 nx[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) nx[i] = __ldg(p + i);
-    }
-    for (uint64_t b = 0; b < nblk; ++b) {
-        uint32_t w[16] = {bswap(nx[0].x), bswap(nx[0].y), bswap(nx[0].z), bswap(nx[0].w), bswap(nx[1].x), bswap(nx[1].y),
-                          bswap(nx[1].z), bswap(nx[1].w), bswap(nx[2].x), bswap(nx[2].y), bswap(nx[2].z), bswap(nx[2].w),
-                          bswap(nx[3].x), bswap(nx[3].y), bswap(nx[3].z), bswap(nx[3].w)};
-        if (b + 1 < nblk) {
+        for (int i = 0; i < 4; ++i) nx[i] = make_uint4(0u, 0u, 0u, 0u);
+        if (nblk) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) nx[i] = __ldg(p + 4 * (b + 1) + i);
+            for (int i = 0; i < 4; ++i) nx[i] = __ldg(p + i);
         }
-        compress(st, w);
-    }
-    // tail: len % 64 bytes (a multiple of 16 here), 0x80, zeros, 64-bit big-endian bit length
-    {
-        const uint32_t rem = (uint32_t)(len & 63u);  // 0, 16, 32 or 48
-        uint32_t w[16];
+        for (uint32_t b = 0; b < iters; ++b) {
+            const uint32_t buf = b & 1u;
+            uint32_t w[16];
+            if (b < nblk) {
+                w[0] = bswap(nx[0].x); w[1] = bswap(nx[0].y); w[2] = bswap(nx[0].z); w[3] = bswap(nx[0].w);
+                w[4] = bswap(nx[1].x); w[5] = bswap(nx[1].y); w[6] = bswap(nx[1].z); w[7] = bswap(nx[1].w);
+                w[8] = bswap(nx[2].x); w[9] = bswap(nx[2].y); w[10] = bswap(nx[2].z); w[11] = bswap(nx[2].w);
+                w[12] = bswap(nx[3].x); w[13] = bswap(nx[3].y); w[14] = bswap(nx[3].z); w[15] = bswap(nx[3].w);
+                if (b + 1u < nblk) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) w[i] = 0u;
-        const uint4 *q = p + 4 * nblk;
+                    for (int i = 0; i < 4; ++i) nx[i] = __ldg(p + 4u * (b + 1u) + i);
+                }
+            } else {
+                // tail block (b == nblk): len % 64 bytes (a multiple of 16 here), 0x80, zeros, 64-bit big-endian bit length;
+                // blocks past it (b > nblk, other lanes still running) are ignored by the round warp
 #pragma unroll
-        for (int i = 0; i < 3; ++i)
-            if ((uint32_t)(16 * (i + 1)) <= rem) {
-                const uint4 v = __ldg(q + i);
-                w[4 * i] = bswap(v.x); w[4 * i + 1] = bswap(v.y); w[4 * i + 2] = bswap(v.z); w[4 * i + 3] = bswap(v.w);
+                for (int i = 0; i < 16; ++i) w[i] = 0u;
+                if (b == nblk) {
+                    const uint32_t rem = (uint32_t)(len & 63u);  // 0, 16, 32 or 48
+                    const uint4 *q = p + 4u * nblk;
+#pragma unroll
+                    for (int i = 0; i < 3; ++i)
+                        if ((uint32_t)(16 * (i + 1)) <= rem) {
+                            const uint4 v = __ldg(q + i);
+                            w[4 * i] = bswap(v.x); w[4 * i + 1] = bswap(v.y); w[4 * i + 2] = bswap(v.z); w[4 * i + 3] = bswap(v.w);
+                        }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        if (rem == (uint32_t)(16 * i)) w[4 * i] = 0x80000000u;
+                    const uint64_t bits = len << 3;  // rem <= 48 < 56: the length always fits in this block
+                    w[14] = (uint32_t)(bits >> 32);
+                    w[15] = (uint32_t)bits;
+                }
             }
+            if (b >= 2u) bar_sync(EMPTY + buf, 64);  // the round warp has finished with this buffer (block b - 2)
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
-            if (rem == (uint32_t)(16 * i)) w[4 * i] = 0x80000000u;
-        // rem <= 48 < 56: the length always fits in this block
-        const uint64_t bits = len << 3;
-        w[14] = (uint32_t)(bits >> 32);
-        w[15] = (uint32_t)bits;
-        compress(st, w);
+            for (int tt = 0; tt < 64; ++tt) {
+                if (tt >= 16) {
+                    const uint32_t w15 = w[(tt + 1) & 15], w2 = w[(tt + 14) & 15];
+                    w[tt & 15] += (ror(w15, 7) ^ ror(w15, 18) ^ (w15 >> 3)) + w[(tt + 9) & 15] + (ror(w2, 17) ^ ror(w2, 19) ^ (w2 >> 10));
+                }
+                Wb[buf][tt][lane] = w[tt & 15] + KT[tt];
+            }
+            __threadfence_block();
+            bar_arrive(FULL + buf, 64);
+        }
+        return;
     }
+
+    // ---------------- round warp ----------------
+    uint32_t st[8] = {0x6a09e667u, 0xbb67ae85u, 0x3c6ef372u, 0xa54ff53au, 0x510e527fu, 0x9b05688cu, 0x1f83d9abu, 0x5be0cd19u};
+    for (uint32_t b = 0; b < iters; ++b) {
+        const uint32_t buf = b & 1u;
+        bar_sync(FULL + buf, 64);
+        uint32_t a = st[0], bb = st[1], c = st[2], d = st[3], e = st[4], ff = st[5], gg = st[6], h = st[7];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) atomicXor(H + (size_t)f * 8u + i, st[i]);
+        for (int tt = 0; tt < 64; ++tt) {
+            const uint32_t t1 = h + (ror(e, 6) ^ ror(e, 11) ^ ror(e, 25)) + (gg ^ (e & (ff ^ gg))) + Wb[buf][tt][lane];
+            const uint32_t t2 = (ror(a, 2) ^ ror(a, 13) ^ ror(a, 22)) + ((a & bb) | (c & (a | bb)));
+            h = gg; gg = ff; ff = e; e = d + t1; d = c; c = bb; bb = a; a = t1 + t2;
+        }
+        if (b <= nblk) {  // this lane's message still has this block
+            st[0] += a; st[1] += bb; st[2] += c; st[3] += d; st[4] += e; st[5] += ff; st[6] += gg; st[7] += h;
+        }
+        if (b + 2u < iters) bar_arrive(EMPTY + buf, 64);  // only when the schedule warp will wait for it
+    }
+    if (live) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) atomicXor(H + (size_t)f * 8u + i, st[i]);
+    }
 }
+
+namespace {
+}  // namespace
 
 // big-endian words -> digest byte order, in place
 __global__ void finish_hash_kernel(uint32_t *H, uint32_t nwords) {
@@ -114,7 +154,7 @@ cudaError_t hash_device(const Geom &g, const uint8_t *d_frames, uint32_t n, uint
     cudaError_t e = cudaMemsetAsync(d_H, 0, m * 32u, st);
     if (e != cudaSuccess) return e;
     const uint32_t total = (uint32_t)(m * (n - band0));
-    sha_bands_kernel<<<(total + 31u) / 32u, 32, 0, st>>>(d_frames, g, n, band0, (uint32_t)m, d_H);
+    sha_bands_kernel<<<(total + 31u) / 32u, 64, 0, st>>>(d_frames, g, n, band0, (uint32_t)m, d_H);
     finish_hash_kernel<<<(unsigned)((m * 8u + 127u) / 128u), 128, 0, st>>>(d_H, (uint32_t)(m * 8u));
     return cudaGetLastError();
 }
