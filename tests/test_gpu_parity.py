@@ -115,6 +115,43 @@ def test_in_place_and_forced_generic(torch_cuda, vb, orc, w, h, nf, generic):
     assert np.array_equal(run_device(torch_cuda, v, ref, D, B, decrypt=True, inplace=True), F)
 
 
+# NEXT-4: the other resolutions of the paper's Tab. VIII: 360 x 240 takes the any-shape
+# kernels (w % 16 != 0), the others the tiled path (720 x 480 and 1280 x 720 with a ragged last column strip)
+@pytest.mark.parametrize("w,h", [(320, 240), (360, 240), (640, 360), (720, 480), (1280, 720)])
+def test_table_viii_resolutions(torch_cuda, vb, orc, w, h):
+    F, D, B = rnd_case(w, h, 2, seed=w + h)
+    v = gpu_ctx(vb, w, h)
+    E = run_device(torch_cuda, v, F, D, B)
+    assert np.array_equal(E[0], orc.confuse_xor(F[0], D[0], B[0]))
+    assert np.array_equal(E[1], orc.confuse_xor(F[1], D[1], B[1]))
+    assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
+
+
+@pytest.mark.parametrize("w,h", [(640, 480), (100, 37)])
+def test_error_locality_without_diffusion(torch_cuda, vb, w, h):
+    """NEXT-4 / pin P10 on the GPU path (cropping and channel noise do not spread): a corrupted
+    ciphertext byte changes at most 2 plaintext bytes, in the same channel, horizontally adjacent (mod w); a cropped
+    rectangle of the ciphertext damages at most that many bytes + one neighbour each."""
+    F, D, B = rnd_case(w, h, 1, seed=3)
+    v = gpu_ctx(vb, w, h)
+    E = run_device(torch_cuda, v, F, D, B)
+    rng = np.random.default_rng(9)
+    for _ in range(8):
+        i, j, c = int(rng.integers(0, h)), int(rng.integers(0, w)), int(rng.integers(0, 3))
+        E2 = E.copy()
+        E2[0, i, j, c] ^= np.uint8(1 + rng.integers(0, 255))
+        P = run_device(torch_cuda, v, E2, D, B, decrypt=True)
+        diff = np.argwhere(P[0] != F[0])
+        assert 1 <= len(diff) <= 2
+        assert set(diff[:, 2]) == {diff[0, 2]} and len(set(diff[:, 0])) == 1
+        if len(diff) == 2:
+            assert (diff[1, 1] - diff[0, 1]) % w in (1, w - 1)
+    E3 = E.copy()
+    E3[0, 5:15, 10:30, :] = 0  # cropping attack (Fig. 8): 10 x 20 pixels blanked
+    P = run_device(torch_cuda, v, E3, D, B, decrypt=True)
+    assert 0 < np.count_nonzero(P[0] != F[0]) <= 2 * 10 * 20 * 3
+
+
 def test_many_frames_per_call_split_into_l2_sized_launches(torch_cuda, vb, orc):
     """More frames than one L2-resident launch holds: the call splits, results unchanged."""
     w, h, nf = 640, 480, 120  # 110.6 MB of frames: two launch pairs (113 + 7 frames)
