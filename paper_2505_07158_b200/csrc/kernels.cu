@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
         const uint64_t pol_in = policy_evict_first();
         // prologue: fill every stage
         for (uint32_t it = 0; it < NS && it < niter; ++it) {
-            const uint32_t blk = blk0 + it * G;
+            const uint32_t blk = INV ? nblocks - 1u - (blk0 + it * G) : blk0 + it * G;
             if (lane < 3 * ROW_RB) {
                 const uint2 pv = row_param(D, g, blk * ROW_RB + pr, pch, INV, poff);
                 par1[it * 16u + pslot] = pv.x;
@@ -196,18 +196,20 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
         }
         uint32_t s = 0, ph = 0;
         for (uint32_t it = 0; it < niter; ++it) {
-            const uint32_t blk = blk0 + it * G;
+            // decrypt walks the blocks last-first: the column pass wrote the last frames last, they are the likeliest in L2
+            const uint32_t blk = INV ? nblocks - 1u - (blk0 + it * G) : blk0 + it * G;
+            const uint32_t blk_next = INV ? blk - NS * G : blk + NS * G;  // only used when it + NS < niter
             const bool refill = it + NS < niter;
             if (refill) {
                 uint2 pnext = make_uint2(0u, 0u);
-                if (lane < 3 * ROW_RB) pnext = row_param(D, g, (blk + NS * G) * ROW_RB + pr, pch, INV, poff);
+                if (lane < 3 * ROW_RB) pnext = row_param(D, g, blk_next * ROW_RB + pr, pch, INV, poff);
                 if (lane == 0) mbar_wait(empty + s, ph);  // phase 1 and phase 2 of block `it` no longer need stage s / its parameters
                 __syncwarp();
                 if (lane < 3 * ROW_RB) { par1[s * 16u + pslot] = pnext.x; par2[s * 16u + pslot] = pnext.y; }
                 __syncwarp();
                 if (lane == 0) {
                     mbar_expect_tx(full + s, blk_bytes);
-                    bulk_g2s_hint(stage0 + s * blk_bytes, src + (size_t)(blk + NS * G) * blk_bytes, blk_bytes, full + s, pol_in);
+                    bulk_g2s_hint(stage0 + s * blk_bytes, src + (size_t)blk_next * blk_bytes, blk_bytes, full + s, pol_in);
                 }
             }
             if (lane == 0) {
@@ -560,10 +562,10 @@ __global__ void __launch_bounds__(NT, MINB)
     const uint32_t f = blockIdx.x / strips_per_frame;
     const uint32_t x0 = (blockIdx.x - f * strips_per_frame) * X;
 
-    pdl_wait();  // the ciphertext may be the previous kernel's output
-    pdl_trigger();
     // look-ahead: thread 0 asks the TMA engine to pull ciphertext and keystream tiles of the strip into L2, one iteration
-    // of rows ahead of the rows the CTA is loading (measured optimum; further ahead is slower)
+    // of rows ahead of the rows the CTA is loading (measured optimum; further ahead is slower).  The first tiles are
+    // requested BEFORE the wait for the previous kernel: an L2 prefetch cannot return stale data (the L2 is the point of
+    // coherence), and it overlaps that kernel's tail.
     constexpr uint32_t CD_AHEAD = 4u * (NT / 32) * (256 / X);
     uint32_t pf_row = 0;
     if (threadIdx.x == 0)
@@ -571,7 +573,7 @@ __global__ void __launch_bounds__(NT, MINB)
             tma_prefetch_2d(&tm_src, (int32_t)x0, (int32_t)(f * h + pf_row));
             tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
         }
-    // one thread per byte column of the strip: t = d_v mod h, the row offset of the column's source
+    // one thread per byte column of the strip: t = d_v mod h, the row offset of the column's source (D is an input)
     if (threadIdx.x >= NT - X) {
         const uint32_t xs = threadIdx.x - (NT - X);
         uint32_t x = x0 + xs;
@@ -580,6 +582,8 @@ __global__ void __launch_bounds__(NT, MINB)
         const uint32_t dv = D[(size_t)f * g.nD + c * (h + g.w) + h + jj];
         ups[xs] = (uint16_t)(dv - __umulhi(dv, h_magic) * h);  // d_v mod h  (h_magic = ceil(2^32 / h), d_v < 2^16)
     }
+    pdl_wait();  // the ciphertext may be the previous kernel's output
+    pdl_trigger();
 
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t sub = lane / LPS, j = lane % LPS;
