@@ -542,37 +542,44 @@ __global__ void __launch_bounds__(NT, MINB)
 // Column pass, decrypt direction: undo the XOR of Algorithm 6, then the vertical shift of
 // Algorithm 5:   dst(i, x) = (src xor B)((i + t_x) mod h, x),   src = F_e row-major, dst row-major (the
 // inverse row pass follows).  Same strip, same T4 layout in shared memory and the same conflict-free
-// gather as the encrypt direction; here the strip is filled by the threads themselves: 64-bit loads of
-// four rows of ciphertext and keystream, XOR, one 4 x 4 byte transpose per word column, 64-bit stores
-// (sub-warps take the byte lanes in the order b ^ (s & 1), so that two sub-warps together cover all banks).
-// In place is safe: the whole strip is in shared memory (barrier) before the first store.
+// gather as the encrypt direction.  The ciphertext strip is brought in by the TMA engine (all of it in
+// flight from the first cycle, no registers held); the threads then turn it into (src xor B) in T4 layout
+// IN PLACE: a lane reads its 8 bytes of four rows, xors the keystream (64-bit global loads, one block ahead,
+// their tiles pulled into L2 by TMA prefetches), transposes 4 x 4 bytes per word column and writes the same
+// 32 bytes back (sub-warps take the rows / byte lanes in the order t ^ (s & 1), so that the two sub-warps of
+// a half warp sit in disjoint banks).
+// In place (dst == src) is safe: the whole strip is in shared memory (barrier) before the first store.
 // ---------------------------------------------------------------------------------------------
 template <int X, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
-    col_dec_kernel(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ CUtensorMap tm_B, const uint8_t *src,
+    col_dec_kernel(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ CUtensorMap tm_B,
                    const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
-                   uint32_t strips_per_frame, uint32_t h_magic, uint32_t box_rows) {
+                   uint32_t strips_per_frame, uint32_t h_magic, uint32_t box_rows, uint32_t pf_rows) {
     extern __shared__ __align__(128) uint8_t S[];
     constexpr uint32_t LPS = X / 8;       // lanes per strip row
     constexpr uint32_t NSUB = 32 / LPS;   // sub-warps per warp
     constexpr uint32_t NW = NT / 32;
     constexpr uint32_t GSTEP = NW * NSUB;  // row groups / row blocks between two iterations of a sub-warp
     const uint32_t h = g.h, rb = g.row_bytes;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(S + (size_t)(h + CE_PAD) * X);
     uint16_t *ups = reinterpret_cast<uint16_t *>(S + (size_t)(h + CE_PAD) * X + 16);  // [X] source row offset per byte column
     const uint32_t f = blockIdx.x / strips_per_frame;
     const uint32_t x0 = (blockIdx.x - f * strips_per_frame) * X;
 
-    // look-ahead: thread 0 asks the TMA engine to pull ciphertext and keystream tiles of the strip into L2, one iteration
-    // of rows ahead of the rows the CTA is loading (measured optimum; further ahead is slower).  The first tiles are
-    // requested BEFORE the wait for the previous kernel: an L2 prefetch cannot return stale data (the L2 is the point of
-    // coherence), and it overlaps that kernel's tail.
-    constexpr uint32_t CD_AHEAD = 4u * (NT / 32) * (256 / X);
+    // keystream look-ahead: thread 0 asks the TMA engine to pull the strip's keystream tiles into L2, CD_AHEAD rows ahead
+    // of the rows the CTA is loading.  The first tiles are requested BEFORE the wait for the previous kernel (the
+    // keystream is never that kernel's output), which overlaps its tail.
+    constexpr uint32_t CD_AHEAD = 2u * 4u * GSTEP;  // two iterations (measured: 1 -> 6.93, 2 -> 6.78, 4 -> 6.95 us per FHD frame)
     uint32_t pf_row = 0;
-    if (threadIdx.x == 0)
-        for (; pf_row < h && pf_row < CD_AHEAD; pf_row += box_rows) {
-            tma_prefetch_2d(&tm_src, (int32_t)x0, (int32_t)(f * h + pf_row));
-            tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
-        }
+    if (threadIdx.x == 0) {
+        for (; pf_row < h && pf_row < CD_AHEAD; pf_row += pf_rows) tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
+        mbar_init(bar, 1);
+        pdl_wait();  // the ciphertext may be the previous kernel's output
+        const uint64_t pol = policy_evict_first();
+        mbar_expect_tx(bar, h * X);
+        const int32_t y0 = (int32_t)(f * h);
+        for (uint32_t r0 = 0; r0 < h; r0 += box_rows) tma_load_2d(S + (size_t)r0 * X, &tm_src, (int32_t)x0, y0 + (int32_t)r0, bar, pol);
+    }
     // one thread per byte column of the strip: t = d_v mod h, the row offset of the column's source (D is an input)
     if (threadIdx.x >= NT - X) {
         const uint32_t xs = threadIdx.x - (NT - X);
@@ -582,7 +589,7 @@ __global__ void __launch_bounds__(NT, MINB)
         const uint32_t dv = D[(size_t)f * g.nD + c * (h + g.w) + h + jj];
         ups[xs] = (uint16_t)(dv - __umulhi(dv, h_magic) * h);  // d_v mod h  (h_magic = ceil(2^32 / h), d_v < 2^16)
     }
-    pdl_wait();  // the ciphertext may be the previous kernel's output
+    pdl_wait();
     pdl_trigger();
 
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -595,63 +602,61 @@ __global__ void __launch_bounds__(NT, MINB)
     const uint32_t rb2 = 2u * rb, rb3 = 3u * rb, rb4 = 4u * rb, rb5 = 5u * rb, rb6 = 6u * rb, rb7 = 7u * rb;
 #define VK_ROWPTR(T, P, OFF) reinterpret_cast<T>(mad_wide_ptr(P, OFF))
 
-    // ---- phase A: (src xor B) -> T4 strip.  Item = (block of 4 rows R, this lane's 8 byte columns)
+    // ---- phase A: strip -> (strip xor B) in T4 layout, in place.  Item = (block of 4 rows R, this lane's 8 byte columns);
+    // step t works on row / byte lane t ^ s1.
+    const uint32_t s1 = sub & 1u;
+    const uint32_t nblk = h >> 2;
+    const uint32_t offs4[4] = {s1 ? rb : 0u, s1 ? 0u : rb, s1 ? rb3 : rb2, s1 ? rb2 : rb3};
+    const uint8_t *pB = Bk + fcol + (size_t)(4u * g0) * rb;
+    uint2 kn[4];
+#pragma unroll
+    for (int t = 0; t < 4; ++t) kn[t] = make_uint2(0u, 0u);
+    if (col_ok && g0 < nblk) {  // keystream of the first block: issued before the strip arrives
+#pragma unroll
+        for (int t = 0; t < 4; ++t) kn[t] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs4[t]));
+    }
+    __syncthreads();    // mbarrier initialised, ups[] complete
+    mbar_wait(bar, 0);  // the ciphertext strip has landed
     if (col_ok) {
-        const uint32_t s1 = sub & 1u;
+        const uint32_t selA = s1 ? 0x1504u : 0x5140u, selB = s1 ? 0x3726u : 0x7362u;  // inputs arrive as rows (t ^ s1)
         const uint32_t selF = s1 ? 0x7632u : 0x5410u, selS = s1 ? 0x5410u : 0x7632u;  // first / second byte lane of a pair
-        const uint32_t nblk = h >> 2;
-        const uint8_t *pS = src + fcol + (size_t)(4u * g0) * rb;
-        const uint8_t *pB = Bk + fcol + (size_t)(4u * g0) * rb;
         const size_t bstep = (size_t)(4u * GSTEP) * rb;
-        // software pipeline: the loads of the next block are in flight while this one is transposed and stored
-        const uint32_t offs[4] = {0u, rb, rb2, rb3};
-        uint2 vn[4], kn[4];
-#pragma unroll
-        for (int r = 0; r < 4; ++r) { vn[r] = make_uint2(0u, 0u); kn[r] = make_uint2(0u, 0u); }
-        if (g0 < nblk) {
-#pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                vn[r] = __ldcs(VK_ROWPTR(const uint2 *, pS, offs[r]));
-                kn[r] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[r]));
-            }
-        }
+        const int32_t d1 = s1 ? -(int32_t)X : (int32_t)X;
         for (uint32_t R4 = g0; R4 < nblk; R4 += GSTEP) {
-            uint2 v[4], k[4];
+            uint2 k[4];
 #pragma unroll
-            for (int r = 0; r < 4; ++r) { v[r] = vn[r]; k[r] = kn[r]; }
-            pS += bstep;
+            for (int t = 0; t < 4; ++t) k[t] = kn[t];
             pB += bstep;
             if (threadIdx.x == 0)
-                for (; pf_row < h && pf_row < 4u * (R4 + GSTEP) + CD_AHEAD; pf_row += box_rows) {
-                    tma_prefetch_2d(&tm_src, (int32_t)x0, (int32_t)(f * h + pf_row));
+                for (; pf_row < h && pf_row < 4u * (R4 + GSTEP) + CD_AHEAD; pf_row += pf_rows)
                     tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
-                }
             if (R4 + GSTEP < nblk) {
 #pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    vn[r] = __ldcs(VK_ROWPTR(const uint2 *, pS, offs[r]));
-                    kn[r] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[r]));
-                }
+                for (int t = 0; t < 4; ++t) kn[t] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs4[t]));
             }
+            uint8_t *ps = S + ((size_t)(4u * R4) * X + 8u * j) + (s1 ? X : 0u);
+            uint2 v[4];
+            v[0] = *reinterpret_cast<const uint2 *>(ps);
+            v[1] = *reinterpret_cast<const uint2 *>(ps + d1);
+            v[2] = *reinterpret_cast<const uint2 *>(ps + 2 * X);
+            v[3] = *reinterpret_cast<const uint2 *>(ps + 2 * X + d1);
 #pragma unroll
-            for (int r = 0; r < 4; ++r) { v[r].x ^= k[r].x; v[r].y ^= k[r].y; }
+            for (int t = 0; t < 4; ++t) { v[t].x ^= k[t].x; v[t].y ^= k[t].y; }
             // two 4 x 4 byte transposes: word column 2j (x) and 2j + 1 (y); outputs in the order b = t ^ s1
             uint32_t lo[4], hi[4];
             {
-                const uint32_t a = __byte_perm(v[0].x, v[1].x, 0x5140), b = __byte_perm(v[0].x, v[1].x, 0x7362);
-                const uint32_t c = __byte_perm(v[2].x, v[3].x, 0x5140), d = __byte_perm(v[2].x, v[3].x, 0x7362);
+                const uint32_t a = __byte_perm(v[0].x, v[1].x, selA), b = __byte_perm(v[0].x, v[1].x, selB);
+                const uint32_t c = __byte_perm(v[2].x, v[3].x, selA), d = __byte_perm(v[2].x, v[3].x, selB);
                 lo[0] = __byte_perm(a, c, selF); lo[1] = __byte_perm(a, c, selS);
                 lo[2] = __byte_perm(b, d, selF); lo[3] = __byte_perm(b, d, selS);
             }
             {
-                const uint32_t a = __byte_perm(v[0].y, v[1].y, 0x5140), b = __byte_perm(v[0].y, v[1].y, 0x7362);
-                const uint32_t c = __byte_perm(v[2].y, v[3].y, 0x5140), d = __byte_perm(v[2].y, v[3].y, 0x7362);
+                const uint32_t a = __byte_perm(v[0].y, v[1].y, selA), b = __byte_perm(v[0].y, v[1].y, selB);
+                const uint32_t c = __byte_perm(v[2].y, v[3].y, selA), d = __byte_perm(v[2].y, v[3].y, selB);
                 hi[0] = __byte_perm(a, c, selF); hi[1] = __byte_perm(a, c, selS);
                 hi[2] = __byte_perm(b, d, selF); hi[3] = __byte_perm(b, d, selS);
             }
             // step t holds byte lane b = t ^ s1: strip row 4 R4 + b, bytes 8j .. 8j+7
-            uint8_t *ps = S + ((size_t)(4u * R4) * X + 8u * j) + (s1 ? X : 0u);
-            const int32_t d1 = s1 ? -(int32_t)X : (int32_t)X;
             *reinterpret_cast<uint2 *>(ps) = make_uint2(lo[0], hi[0]);
             *reinterpret_cast<uint2 *>(ps + d1) = make_uint2(lo[1], hi[1]);
             *reinterpret_cast<uint2 *>(ps + 2 * X) = make_uint2(lo[2], hi[2]);
@@ -946,11 +951,11 @@ static cudaError_t launch_col_dec(const Geom &g, const Plan &p, const uint8_t *s
                                   size_t n, uint8_t *dst, cudaStream_t st) {
     alignas(64) CUtensorMap tm_src, tm_B;
     const uint32_t pbox = 64;  // look-ahead tile height (rows)
-    if (!make_tmap(p, g, src, n, pbox, &tm_src) || !make_tmap(p, g, B, n, pbox, &tm_B)) return cudaErrorInvalidValue;
+    if (!make_tmap(p, g, src, n, p.box_rows, &tm_src) || !make_tmap(p, g, B, n, pbox, &tm_B)) return cudaErrorInvalidValue;
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
-#define VK_COLD(X, NT, MINB)                                                                                              \
-    return launch_pdl(col_dec_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_src, tm_B, src, B, dst, D, g,           \
-                      (uint32_t)p.strips_per_frame, p.h_magic, pbox)
+#define VK_COLD(X, NT, MINB)                                                                                         \
+    return launch_pdl(col_dec_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_src, tm_B, B, dst, D, g,           \
+                      (uint32_t)p.strips_per_frame, p.h_magic, p.box_rows, pbox)
     if (p.col_ctas_per_sm == 3) {
         if (p.strip_bytes == 64) VK_COLD(64, 256, 3);
         else VK_COLD(32, 256, 3);
