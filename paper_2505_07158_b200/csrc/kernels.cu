@@ -94,9 +94,10 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 //            plane words; the chunk is stored already rotated by the whole-chunk part of the distance;
 //   phase 2 (one item = a quad of 4 pixels, all 4 rows, all 3 channels): 12 funnel shifts, then either three
 //            4 x 4 byte transposes (T4: the word at (row 4R + (x & 3), word column x >> 2) holds byte column x
-//            of rows 4R .. 4R+3) or the re-interleave to row-major; the result overwrites the stage.
-// Synchronisation: full[s] (mbarrier, transaction bytes) copy warp -> compute threads; done[s] (mbarrier,
-// one arrival) compute threads -> copy warp; named barrier 1 among the compute threads.
+//            of rows 4R .. 4R+3) or the re-interleave to row-major; the result goes to one output buffer.
+// Synchronisation: full[s] (mbarrier, transaction bytes) copy warp -> compute threads; empty[s] (one arrival)
+// compute threads -> copy warp once phase 1 has consumed the stage; ofull / ofree (one arrival each) hand the
+// output buffer to the copy warp's bulk store and back; named barrier 1 among the compute threads.
 // In place (dst == src) is safe: a block is read completely before it is written.
 // ---------------------------------------------------------------------------------------------
 constexpr int ROW_RB = 4;       // rows per block

@@ -2,9 +2,10 @@
 // frame of a batch and H = xor_m h_m, on the frames that were uploaded for the cipher kernels anyway.
 //
 // SHA-256 (FIPS 180-4) is serial inside a message, so the parallelism is one message per (frame, band): n x batch
-// independent message streams (256 at n = 32, batch = 8), 32 messages per CTA so that the CTAs spread over as many SMs as
-// possible.  A band is walked 64 bytes at a time with 128-bit loads, the next block in flight while the current one is
-// processed, the tail padded as the standard says, and the digest xor-ed into the frame's H with eight atomicXor.
+// independent message streams (256 at n = 32, batch = 8), 32 messages per CTA (two warps, see below) so that the CTAs
+// spread over as many SMs as possible.  A band is walked 64 bytes at a time with 128-bit loads, the next block in flight
+// while the current one is processed, the tail padded as the standard says, and the digest xor-ed into the frame's H
+// with eight atomicXor.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -137,9 +138,6 @@ __global__ void __launch_bounds__(64) sha_bands_kernel(const uint8_t *__restrict
         for (int i = 0; i < 8; ++i) atomicXor(H + (size_t)f * 8u + i, st[i]);
     }
 }
-
-namespace {
-}  // namespace
 
 // big-endian words -> digest byte order, in place
 __global__ void finish_hash_kernel(uint32_t *H, uint32_t nwords) {
