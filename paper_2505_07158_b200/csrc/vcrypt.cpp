@@ -92,6 +92,18 @@ int cuda_fail(vcrypt_ctx *c, cudaError_t e, const char *what) {
         if (e__ != cudaSuccess) return cuda_fail((ctx), e__, #call); \
     } while (0)
 
+// No exception may cross the C ABI (include/vcrypt.h): host allocations inside an entry point become VCRYPT_E_NOMEM.
+template <class F>
+int guarded(F &&body) noexcept {
+    try {
+        return body();
+    } catch (const std::bad_alloc &) {
+        return VCRYPT_E_NOMEM;
+    } catch (...) {
+        return VCRYPT_E_ARG;
+    }
+}
+
 bool is_pinned(const void *p) {
     cudaPointerAttributes a;
     if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
@@ -410,68 +422,76 @@ int chain_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, do
 }  // namespace
 
 extern "C" int vcrypt_frame_hash(vcrypt_ctx *c, const uint8_t *frame, uint8_t *H_out) {
-    if (!c || !frame || !H_out) return VCRYPT_E_ARG;
-    hash_frames(c, frame, 1, H_out, c->p.n_workers);
-    return VCRYPT_OK;
+    return guarded([&]() -> int {
+        if (!c || !frame || !H_out) return VCRYPT_E_ARG;
+        hash_frames(c, frame, 1, H_out, c->p.n_workers);
+        return VCRYPT_OK;
+    });
 }
 
 extern "C" int vcrypt_derive(vcrypt_ctx *c, const uint8_t *hash, uint16_t *D_out, uint8_t *B_out) {
-    if (!c || !hash || !D_out || !B_out) return VCRYPT_E_ARG;
-    double S[4];
-    std::memcpy(S, c->S, sizeof S);
-    const int rc = derive_frames(c, S, hash, 1, D_out, B_out);
-    if (rc != VCRYPT_OK) return rc;
-    std::memcpy(c->S, S, sizeof S);
-    c->frames_done += 1;
-    return VCRYPT_OK;
+    return guarded([&]() -> int {
+        if (!c || !hash || !D_out || !B_out) return VCRYPT_E_ARG;
+        double S[4];
+        std::memcpy(S, c->S, sizeof S);
+        const int rc = derive_frames(c, S, hash, 1, D_out, B_out);
+        if (rc != VCRYPT_OK) return rc;
+        std::memcpy(c->S, S, sizeof S);
+        c->frames_done += 1;
+        return VCRYPT_OK;
+    });
 }
 
 extern "C" int vcrypt_frame_hash_device(vcrypt_ctx *c, const void *d_frames, size_t n, uint8_t *hashes_out, void *stream) {
-    if (!c || !d_frames || !hashes_out || n == 0) return VCRYPT_E_ARG;
-    if (!c->cuda) return VCRYPT_E_CUDA;
-    if ((((uintptr_t)d_frames) & 15u) || c->g.row_bytes % 16u != 0) return VCRYPT_E_SHAPE;
-    VC_CUDA(c, cudaSetDevice(c->device));
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    uint32_t *d_H = nullptr;
-    cudaError_t e = cudaMalloc(&d_H, n * 32u);
-    if (e == cudaSuccess) e = vk::hash_device(c->g, static_cast<const uint8_t *>(d_frames), c->p.n_workers, 0, n, d_H, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(hashes_out, d_H, n * 32u, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (d_H) cudaFree(d_H);
-    if (e != cudaSuccess) return cuda_fail(c, e, "device hashing");
-    return VCRYPT_OK;
+    return guarded([&]() -> int {
+        if (!c || !d_frames || !hashes_out || n == 0) return VCRYPT_E_ARG;
+        if (!c->cuda) return VCRYPT_E_CUDA;
+        if ((((uintptr_t)d_frames) & 15u) || c->g.row_bytes % 16u != 0) return VCRYPT_E_SHAPE;
+        VC_CUDA(c, cudaSetDevice(c->device));
+        cudaStream_t st = static_cast<cudaStream_t>(stream);
+        uint32_t *d_H = nullptr;
+        cudaError_t e = cudaMalloc(&d_H, n * 32u);
+        if (e == cudaSuccess) e = vk::hash_device(c->g, static_cast<const uint8_t *>(d_frames), c->p.n_workers, 0, n, d_H, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(hashes_out, d_H, n * 32u, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (d_H) cudaFree(d_H);
+        if (e != cudaSuccess) return cuda_fail(c, e, "device hashing");
+        return VCRYPT_OK;
+    });
 }
 
 extern "C" int vcrypt_derive_device(vcrypt_ctx *c, const uint8_t *hash, void *d_D, void *d_B, void *stream) {
-    if (!c || !hash || !d_D || !d_B) return VCRYPT_E_ARG;
-    if (!c->cuda) return VCRYPT_E_CUDA;
-    if ((((uintptr_t)d_B) & 7u) || (((uintptr_t)d_D) & 1u)) return VCRYPT_E_ARG;
-    VC_CUDA(c, cudaSetDevice(c->device));
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t irb = 2u * (size_t)c->p.n_workers * 4u * sizeof(double);
-    double S[4];
-    std::memcpy(S, c->S, sizeof S);
-    std::vector<double> IR(2u * (size_t)c->p.n_workers * 4u);
-    int rc = chain_frames(c, S, hash, 1, IR.data());
-    if (rc != VCRYPT_OK) return rc;
-    double *d_IR = nullptr;
-    uint32_t *d_status = nullptr, h_status = 0;
-    cudaError_t e = cudaMalloc(&d_IR, irb);
-    if (e == cudaSuccess) e = cudaMalloc(&d_status, sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_IR, IR.data(), irb, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(d_status, 0, sizeof(uint32_t), st);
-    if (e == cudaSuccess)
-        e = vk::derive_device(c->g, d_IR, c->p.gamma, c->p.n_workers, 1, static_cast<uint16_t *>(d_D), static_cast<uint8_t *>(d_B),
-                              d_status, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_status, d_status, sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (d_IR) cudaFree(d_IR);
-    if (d_status) cudaFree(d_status);
-    if (e != cudaSuccess) return cuda_fail(c, e, "device derivation");
-    if (h_status) return VCRYPT_E_STATE;
-    std::memcpy(c->S, S, sizeof S);
-    c->frames_done += 1;
-    return VCRYPT_OK;
+    return guarded([&]() -> int {
+        if (!c || !hash || !d_D || !d_B) return VCRYPT_E_ARG;
+        if (!c->cuda) return VCRYPT_E_CUDA;
+        if ((((uintptr_t)d_B) & 7u) || (((uintptr_t)d_D) & 1u)) return VCRYPT_E_ARG;
+        VC_CUDA(c, cudaSetDevice(c->device));
+        cudaStream_t st = static_cast<cudaStream_t>(stream);
+        const size_t irb = 2u * (size_t)c->p.n_workers * 4u * sizeof(double);
+        double S[4];
+        std::memcpy(S, c->S, sizeof S);
+        std::vector<double> IR(2u * (size_t)c->p.n_workers * 4u);
+        int rc = chain_frames(c, S, hash, 1, IR.data());
+        if (rc != VCRYPT_OK) return rc;
+        double *d_IR = nullptr;
+        uint32_t *d_status = nullptr, h_status = 0;
+        cudaError_t e = cudaMalloc(&d_IR, irb);
+        if (e == cudaSuccess) e = cudaMalloc(&d_status, sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_IR, IR.data(), irb, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(d_status, 0, sizeof(uint32_t), st);
+        if (e == cudaSuccess)
+            e = vk::derive_device(c->g, d_IR, c->p.gamma, c->p.n_workers, 1, static_cast<uint16_t *>(d_D), static_cast<uint8_t *>(d_B),
+                                  d_status, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&h_status, d_status, sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (d_IR) cudaFree(d_IR);
+        if (d_status) cudaFree(d_status);
+        if (e != cudaSuccess) return cuda_fail(c, e, "device derivation");
+        if (h_status) return VCRYPT_E_STATE;
+        std::memcpy(c->S, S, sizeof S);
+        c->frames_done += 1;
+        return VCRYPT_OK;
+    });
 }
 
 // =====================================================================================================
@@ -496,12 +516,16 @@ static int device_call(vcrypt_ctx *c, bool decrypt, const void *d_in, const void
 
 extern "C" int vcrypt_encrypt_device(vcrypt_ctx *c, const void *d_frames, const void *d_D, const void *d_B, size_t n,
                                      void *d_cipher, void *stream) {
-    return device_call(c, false, d_frames, d_D, d_B, n, d_cipher, stream);
+    return guarded([&]() -> int {
+        return device_call(c, false, d_frames, d_D, d_B, n, d_cipher, stream);
+    });
 }
 
 extern "C" int vcrypt_decrypt_device(vcrypt_ctx *c, const void *d_cipher, const void *d_D, const void *d_B, size_t n,
                                      void *d_plain, void *stream) {
-    return device_call(c, true, d_cipher, d_D, d_B, n, d_plain, stream);
+    return guarded([&]() -> int {
+        return device_call(c, true, d_cipher, d_D, d_B, n, d_plain, stream);
+    });
 }
 
 // =====================================================================================================
@@ -523,125 +547,133 @@ double entropy_bits(const uint32_t *z, double total) {  // Eq. 10
 
 extern "C" int vcrypt_frame_stats_device(vcrypt_ctx *c, const void *d_frames, size_t n, vcrypt_frame_stats *out, uint32_t *hist_out,
                                          void *stream) {
-    if (!c || !d_frames || !out || n == 0) return VCRYPT_E_ARG;
-    if (!c->cuda) return VCRYPT_E_CUDA;
-    VC_CUDA(c, cudaSetDevice(c->device));
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    uint32_t *d_hist = nullptr;
-    unsigned long long *d_pairs = nullptr;
-    std::vector<uint32_t> hist(n * 768u);
-    std::vector<unsigned long long> pairs(n * 45u);
-    cudaError_t e = cudaMalloc(&d_hist, n * 768u * sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMalloc(&d_pairs, n * 45u * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = vk::stats_device(c->g, static_cast<const uint8_t *>(d_frames), n, d_hist, d_pairs, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(hist.data(), d_hist, hist.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(pairs.data(), d_pairs, pairs.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (d_hist) cudaFree(d_hist);
-    if (d_pairs) cudaFree(d_pairs);
-    if (e != cudaSuccess) return cuda_fail(c, e, "frame statistics");
-    const double N = (double)c->g.w * (double)c->g.h;
-    const uint64_t w = c->g.w, h = c->g.h;
-    const double npairs[3] = {(double)((w - 1) * h), (double)(w * (h - 1)), (double)((w - 1) * (h - 1))};
-    for (size_t f = 0; f < n; ++f) {
-        vcrypt_frame_stats &o = out[f];
-        for (int ch = 0; ch < 3; ++ch) {
-            const uint32_t *z = hist.data() + f * 768u + ch * 256u;
-            double s1 = 0.0, s2 = 0.0, chi = 0.0;
-            const double ex = N / 256.0;
-            for (int i = 0; i < 256; ++i) {
-                s1 += (double)z[i];
-                s2 += (double)z[i] * (double)z[i];
-                chi += ((double)z[i] - ex) * ((double)z[i] - ex) / ex;
-            }
-            // Eq. 4: (1/256^2) sum_i sum_j (z_i - z_j)^2 / 2 = (256 sum z^2 - (sum z)^2) / 256^2
-            o.hist_variance[ch] = (256.0 * s2 - s1 * s1) / 65536.0;
-            o.chi2[ch] = chi;
-            o.entropy[ch] = entropy_bits(z, N);
-            for (int d = 0; d < 3; ++d) {
-                const unsigned long long *p = pairs.data() + f * 45u + (ch * 3 + d) * 5;
-                const double M = npairs[d];
-                if (M <= 0.0) { o.corr[ch][d] = std::nan(""); continue; }
-                // Eq. 6-9 from the exact sums: cov = E[xy] - E[x]E[y], D(x) = E[x^2] - E[x]^2 (integer numerators)
-                const long double sx = (long double)p[0], sy = (long double)p[1], sxy = (long double)p[2], sxx = (long double)p[3],
-                                  syy = (long double)p[4], m = (long double)M;
-                const long double cov = m * sxy - sx * sy, dx = m * sxx - sx * sx, dy = m * syy - sy * sy;
-                o.corr[ch][d] = (dx > 0 && dy > 0) ? (double)(cov / std::sqrt(dx * dy)) : std::nan("");
+    return guarded([&]() -> int {
+        if (!c || !d_frames || !out || n == 0) return VCRYPT_E_ARG;
+        if (!c->cuda) return VCRYPT_E_CUDA;
+        VC_CUDA(c, cudaSetDevice(c->device));
+        cudaStream_t st = static_cast<cudaStream_t>(stream);
+        uint32_t *d_hist = nullptr;
+        unsigned long long *d_pairs = nullptr;
+        std::vector<uint32_t> hist(n * 768u);
+        std::vector<unsigned long long> pairs(n * 45u);
+        cudaError_t e = cudaMalloc(&d_hist, n * 768u * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMalloc(&d_pairs, n * 45u * sizeof(unsigned long long));
+        if (e == cudaSuccess) e = vk::stats_device(c->g, static_cast<const uint8_t *>(d_frames), n, d_hist, d_pairs, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(hist.data(), d_hist, hist.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(pairs.data(), d_pairs, pairs.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (d_hist) cudaFree(d_hist);
+        if (d_pairs) cudaFree(d_pairs);
+        if (e != cudaSuccess) return cuda_fail(c, e, "frame statistics");
+        const double N = (double)c->g.w * (double)c->g.h;
+        const uint64_t w = c->g.w, h = c->g.h;
+        const double npairs[3] = {(double)((w - 1) * h), (double)(w * (h - 1)), (double)((w - 1) * (h - 1))};
+        for (size_t f = 0; f < n; ++f) {
+            vcrypt_frame_stats &o = out[f];
+            for (int ch = 0; ch < 3; ++ch) {
+                const uint32_t *z = hist.data() + f * 768u + ch * 256u;
+                double s1 = 0.0, s2 = 0.0, chi = 0.0;
+                const double ex = N / 256.0;
+                for (int i = 0; i < 256; ++i) {
+                    s1 += (double)z[i];
+                    s2 += (double)z[i] * (double)z[i];
+                    chi += ((double)z[i] - ex) * ((double)z[i] - ex) / ex;
+                }
+                // Eq. 4: (1/256^2) sum_i sum_j (z_i - z_j)^2 / 2 = (256 sum z^2 - (sum z)^2) / 256^2
+                o.hist_variance[ch] = (256.0 * s2 - s1 * s1) / 65536.0;
+                o.chi2[ch] = chi;
+                o.entropy[ch] = entropy_bits(z, N);
+                for (int d = 0; d < 3; ++d) {
+                    const unsigned long long *p = pairs.data() + f * 45u + (ch * 3 + d) * 5;
+                    const double M = npairs[d];
+                    if (M <= 0.0) { o.corr[ch][d] = std::nan(""); continue; }
+                    // Eq. 6-9 from the exact sums: cov = E[xy] - E[x]E[y], D(x) = E[x^2] - E[x]^2 (integer numerators)
+                    const long double sx = (long double)p[0], sy = (long double)p[1], sxy = (long double)p[2], sxx = (long double)p[3],
+                                      syy = (long double)p[4], m = (long double)M;
+                    const long double cov = m * sxy - sx * sy, dx = m * sxx - sx * sx, dy = m * syy - sy * sy;
+                    o.corr[ch][d] = (dx > 0 && dy > 0) ? (double)(cov / std::sqrt(dx * dy)) : std::nan("");
+                }
             }
         }
-    }
-    if (hist_out) std::memcpy(hist_out, hist.data(), hist.size() * sizeof(uint32_t));
-    return VCRYPT_OK;
+        if (hist_out) std::memcpy(hist_out, hist.data(), hist.size() * sizeof(uint32_t));
+        return VCRYPT_OK;
+    });
 }
 
 extern "C" int vcrypt_npcr_uaci_device(vcrypt_ctx *c, const void *d_a, const void *d_b, size_t n, double *npcr, double *uaci,
                                        void *stream) {
-    if (!c || !d_a || !d_b || !npcr || !uaci || n == 0) return VCRYPT_E_ARG;
-    if (!c->cuda) return VCRYPT_E_CUDA;
-    VC_CUDA(c, cudaSetDevice(c->device));
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    unsigned long long *d_out = nullptr;
-    std::vector<unsigned long long> r(n * 6u);
-    cudaError_t e = cudaMalloc(&d_out, r.size() * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = vk::diff_device(c->g, static_cast<const uint8_t *>(d_a), static_cast<const uint8_t *>(d_b), n, d_out, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(r.data(), d_out, r.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (d_out) cudaFree(d_out);
-    if (e != cudaSuccess) return cuda_fail(c, e, "NPCR / UACI");
-    const double N = (double)c->g.w * (double)c->g.h;
-    for (size_t f = 0; f < n; ++f) {
-        unsigned long long ne = 0, ad = 0;
-        for (int ch = 0; ch < 3; ++ch) {
-            const unsigned long long a = r[f * 6u + 2 * ch], b = r[f * 6u + 2 * ch + 1];
-            ne += a;
-            ad += b;
-            npcr[4 * f + 1 + ch] = 100.0 * (double)a / N;            // Eq. 14, 16
-            uaci[4 * f + 1 + ch] = 100.0 * (double)b / (N * 255.0);  // Eq. 15
+    return guarded([&]() -> int {
+        if (!c || !d_a || !d_b || !npcr || !uaci || n == 0) return VCRYPT_E_ARG;
+        if (!c->cuda) return VCRYPT_E_CUDA;
+        VC_CUDA(c, cudaSetDevice(c->device));
+        cudaStream_t st = static_cast<cudaStream_t>(stream);
+        unsigned long long *d_out = nullptr;
+        std::vector<unsigned long long> r(n * 6u);
+        cudaError_t e = cudaMalloc(&d_out, r.size() * sizeof(unsigned long long));
+        if (e == cudaSuccess) e = vk::diff_device(c->g, static_cast<const uint8_t *>(d_a), static_cast<const uint8_t *>(d_b), n, d_out, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(r.data(), d_out, r.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (d_out) cudaFree(d_out);
+        if (e != cudaSuccess) return cuda_fail(c, e, "NPCR / UACI");
+        const double N = (double)c->g.w * (double)c->g.h;
+        for (size_t f = 0; f < n; ++f) {
+            unsigned long long ne = 0, ad = 0;
+            for (int ch = 0; ch < 3; ++ch) {
+                const unsigned long long a = r[f * 6u + 2 * ch], b = r[f * 6u + 2 * ch + 1];
+                ne += a;
+                ad += b;
+                npcr[4 * f + 1 + ch] = 100.0 * (double)a / N;            // Eq. 14, 16
+                uaci[4 * f + 1 + ch] = 100.0 * (double)b / (N * 255.0);  // Eq. 15
+            }
+            npcr[4 * f] = 100.0 * (double)ne / (3.0 * N);
+            uaci[4 * f] = 100.0 * (double)ad / (3.0 * N * 255.0);
         }
-        npcr[4 * f] = 100.0 * (double)ne / (3.0 * N);
-        uaci[4 * f] = 100.0 * (double)ad / (3.0 * N * 255.0);
-    }
-    return VCRYPT_OK;
+        return VCRYPT_OK;
+    });
 }
 
 extern "C" int vcrypt_local_entropy_device(vcrypt_ctx *c, const void *d_frames, size_t n, const uint32_t *xy, uint32_t k, uint32_t side,
                                            double *out, void *stream) {
-    if (!c || !d_frames || !xy || !out || n == 0 || k == 0 || side == 0) return VCRYPT_E_ARG;
-    if (!c->cuda) return VCRYPT_E_CUDA;
-    for (uint32_t b = 0; b < k; ++b)
-        if ((uint64_t)xy[2 * b] + side > c->g.w || (uint64_t)xy[2 * b + 1] + side > c->g.h) return VCRYPT_E_ARG;
-    VC_CUDA(c, cudaSetDevice(c->device));
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    uint32_t *d_xy = nullptr, *d_bh = nullptr;
-    std::vector<uint32_t> bh(n * k * 768u);
-    cudaError_t e = cudaMalloc(&d_xy, 2u * k * sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMalloc(&d_bh, bh.size() * sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_xy, xy, 2u * k * sizeof(uint32_t), cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = vk::block_hist_device(c->g, static_cast<const uint8_t *>(d_frames), n, d_xy, k, side, d_bh, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(bh.data(), d_bh, bh.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (d_xy) cudaFree(d_xy);
-    if (d_bh) cudaFree(d_bh);
-    if (e != cudaSuccess) return cuda_fail(c, e, "local entropy");
-    const double TB = (double)side * (double)side;
-    for (size_t f = 0; f < n; ++f)
-        for (int ch = 0; ch < 3; ++ch) {
-            double acc = 0.0;
-            for (uint32_t b = 0; b < k; ++b) acc += entropy_bits(bh.data() + ((f * k + b) * 3u + ch) * 256u, TB);
-            out[3 * f + ch] = acc / (double)k;  // Eq. 11
-        }
-    return VCRYPT_OK;
+    return guarded([&]() -> int {
+        if (!c || !d_frames || !xy || !out || n == 0 || k == 0 || side == 0) return VCRYPT_E_ARG;
+        if (!c->cuda) return VCRYPT_E_CUDA;
+        for (uint32_t b = 0; b < k; ++b)
+            if ((uint64_t)xy[2 * b] + side > c->g.w || (uint64_t)xy[2 * b + 1] + side > c->g.h) return VCRYPT_E_ARG;
+        VC_CUDA(c, cudaSetDevice(c->device));
+        cudaStream_t st = static_cast<cudaStream_t>(stream);
+        uint32_t *d_xy = nullptr, *d_bh = nullptr;
+        std::vector<uint32_t> bh(n * k * 768u);
+        cudaError_t e = cudaMalloc(&d_xy, 2u * k * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMalloc(&d_bh, bh.size() * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_xy, xy, 2u * k * sizeof(uint32_t), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = vk::block_hist_device(c->g, static_cast<const uint8_t *>(d_frames), n, d_xy, k, side, d_bh, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(bh.data(), d_bh, bh.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (d_xy) cudaFree(d_xy);
+        if (d_bh) cudaFree(d_bh);
+        if (e != cudaSuccess) return cuda_fail(c, e, "local entropy");
+        const double TB = (double)side * (double)side;
+        for (size_t f = 0; f < n; ++f)
+            for (int ch = 0; ch < 3; ++ch) {
+                double acc = 0.0;
+                for (uint32_t b = 0; b < k; ++b) acc += entropy_bits(bh.data() + ((f * k + b) * 3u + ch) * 256u, TB);
+                out[3 * f + ch] = acc / (double)k;  // Eq. 11
+            }
+        return VCRYPT_OK;
+    });
 }
 
 extern "C" int vcrypt_memory_probe(vcrypt_ctx *c, int which, size_t frames, int reps, double *us_per_rep) {
-    if (!c || !us_per_rep || which < 0 || which > 2 || frames == 0 || reps < 1) return VCRYPT_E_ARG;
-    if (!c->cuda) return VCRYPT_E_CUDA;
-    VC_CUDA(c, cudaSetDevice(c->device));
-    const cudaError_t e = vk::memory_probe(c->g, which, frames, reps, nullptr, us_per_rep);
-    if (e == cudaErrorInvalidValue) return VCRYPT_E_ARG;
-    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return VCRYPT_E_NOMEM; }
-    if (e != cudaSuccess) return cuda_fail(c, e, "memory probe");
-    return VCRYPT_OK;
+    return guarded([&]() -> int {
+        if (!c || !us_per_rep || which < 0 || which > 2 || frames == 0 || reps < 1) return VCRYPT_E_ARG;
+        if (!c->cuda) return VCRYPT_E_CUDA;
+        VC_CUDA(c, cudaSetDevice(c->device));
+        const cudaError_t e = vk::memory_probe(c->g, which, frames, reps, nullptr, us_per_rep);
+        if (e == cudaErrorInvalidValue) return VCRYPT_E_ARG;
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return VCRYPT_E_NOMEM; }
+        if (e != cudaSuccess) return cuda_fail(c, e, "memory probe");
+        return VCRYPT_OK;
+    });
 }
 
 // =====================================================================================================
@@ -779,10 +811,14 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
 
 extern "C" int vcrypt_encrypt_frames(vcrypt_ctx *c, const uint8_t *frames, size_t n, uint8_t *cipher_out,
                                      uint8_t *hashes_out) {
-    return run_frames(c, false, frames, nullptr, n, cipher_out, hashes_out);
+    return guarded([&]() -> int {
+        return run_frames(c, false, frames, nullptr, n, cipher_out, hashes_out);
+    });
 }
 
 extern "C" int vcrypt_decrypt_frames(vcrypt_ctx *c, const uint8_t *cipher, const uint8_t *hashes, size_t n,
                                      uint8_t *plain_out) {
-    return run_frames(c, true, cipher, hashes, n, plain_out, nullptr);
+    return guarded([&]() -> int {
+        return run_frames(c, true, cipher, hashes, n, plain_out, nullptr);
+    });
 }
