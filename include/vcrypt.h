@@ -80,6 +80,12 @@ typedef struct vcrypt_params {
     uint32_t device_hash_bands; /* with VCRYPT_FLAG_DEVICE_HASH: how many of the n row bands of every frame the GPU
                                hashes (the last ones; the host threads hash the others at the same time);
                                0 or values above n -> all n.  Does not affect results                          */
+    uint32_t pipe_frames;   /* vcrypt_{en,de}crypt_device on a resident clip: frames per launch pair when a call brings
+                               at least 2 x pipe_frames frames; such a call alternates its launch pairs over
+                               `pipe_streams` streams (the caller's + internal ones forked from and joined into it),
+                               so that one pair's column pass overlaps the next pair's row pass.  0 -> from the frame
+                               size (about 37 MB of frames per pair).  Does not affect results                     */
+    uint32_t pipe_streams;  /* 0 -> 2; 1 -> off (every launch on the caller's stream); at most 4                    */
 } vcrypt_params;
 
 /* Algorithm 1 set-up (PAPER.md:85 steps 1-2): validates the parameters, whitens the key (reading Q5 of

@@ -21,7 +21,8 @@ class Params(C.Structure):
     _fields_ = [("x0", C.c_double), ("y0", C.c_double), ("z0", C.c_double), ("w0", C.c_double),
                 ("gamma", C.c_double), ("n_workers", C.c_uint32), ("width", C.c_uint32), ("height", C.c_uint32),
                 ("batch", C.c_uint32), ("n_streams", C.c_uint32), ("host_threads", C.c_uint32),
-                ("flags", C.c_uint32), ("device", C.c_int32), ("device_hash_bands", C.c_uint32)]
+                ("flags", C.c_uint32), ("device", C.c_int32), ("device_hash_bands", C.c_uint32),
+                ("pipe_frames", C.c_uint32), ("pipe_streams", C.c_uint32)]
 
 
 class FrameStats(C.Structure):
@@ -105,14 +106,15 @@ class Vcrypt:
     """One vcrypt_ctx.  Method names follow the C calls without the vcrypt_ prefix."""
 
     def __init__(self, key, gamma: float, n_workers: int, width: int, height: int, batch: int = 0,
-                 n_streams: int = 0, host_threads: int = 0, flags: int = 0, device: int = -1, device_hash_bands: int = 0):
+                 n_streams: int = 0, host_threads: int = 0, flags: int = 0, device: int = -1, device_hash_bands: int = 0,
+                 pipe_frames: int = 0, pipe_streams: int = 0):
         self.L = lib()
         self.w, self.h, self.n = int(width), int(height), int(n_workers)
         self.frame_bytes = 3 * self.w * self.h
         self.nD = 3 * (self.w + self.h)
         x0, y0, z0, w0 = (float(v) for v in key)
         self.params = Params(x0, y0, z0, w0, float(gamma), n_workers, width, height, batch, n_streams,
-                             host_threads, flags, device, device_hash_bands)
+                             host_threads, flags, device, device_hash_bands, pipe_frames, pipe_streams)
         self._p = _vp()
         rc = self.L.vcrypt_init(C.byref(self._p), C.byref(self.params))
         if rc != OK:

@@ -71,6 +71,12 @@ struct vcrypt_ctx {
     std::vector<double> IR;               // batch x 2n x 4
     std::vector<vh::WorkerSlice> slices;  // batch x n
     std::vector<uint8_t> subhash;         // batch x n x 32
+    // resident-clip schedule of the *_device calls (launch pairs alternating over streams): see launch_cipher
+    static constexpr int kPipeMax = 4;
+    size_t pipe_frames = 0;
+    int pipe_streams = 2;
+    cudaStream_t pipe_st[kPipeMax - 1] = {nullptr, nullptr, nullptr};
+    cudaEvent_t pipe_fork = nullptr, pipe_join[kPipeMax - 1] = {nullptr, nullptr, nullptr};
     // generic-path scratch for in-place calls
     uint8_t *d_scratch = nullptr;
     size_t scratch_bytes = 0;
@@ -199,8 +205,47 @@ int launch_cipher(vcrypt_ctx *c, bool decrypt, const uint8_t *src, const uint16_
     cudaError_t e;
     const bool aligned = ((((uintptr_t)src) | ((uintptr_t)dst) | ((uintptr_t)B)) & 15u) == 0;
     if (c->plan.tiled && aligned && !(c->p.flags & VCRYPT_FLAG_FORCE_GENERIC)) {
-        e = decrypt ? vk::decrypt_tiled(c->g, c->plan, src, D, B, n, dst, st, &launches)
-                    : vk::encrypt_tiled(c->g, c->plan, src, D, B, n, dst, st, &launches);
+        const size_t pf = c->pipe_frames;
+        if (c->pipe_streams >= 2 && n >= 2 * pf) {
+            // Resident clip.  The two passes of a launch pair stress different parts of the memory system (the row pass
+            // reads DRAM and fills L2, the column pass's CTAs first pull their strips out of L2 and then stream DRAM), and
+            // inside one stream a pass only starts when its predecessor has drained.  Frames are independent, so the
+            // pairs go round-robin over `pipe_streams` streams -- the caller's and internal ones that fork from it here
+            // and join it below: the column pass of one pair overlaps the row pass of the next.  Pairs are kept small
+            // enough for the intermediates of all streams to stay in L2 together (measured).
+            const int S = c->pipe_streams;
+            e = cudaSuccess;
+            for (int i = 0; i + 1 < S && e == cudaSuccess; ++i) {
+                if (!c->pipe_st[i]) e = cudaStreamCreateWithFlags(&c->pipe_st[i], cudaStreamNonBlocking);
+                if (e == cudaSuccess && !c->pipe_join[i]) e = cudaEventCreateWithFlags(&c->pipe_join[i], cudaEventDisableTiming);
+            }
+            if (e == cudaSuccess && !c->pipe_fork) e = cudaEventCreateWithFlags(&c->pipe_fork, cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventRecord(c->pipe_fork, st);
+            for (int i = 0; i + 1 < S && e == cudaSuccess; ++i) e = cudaStreamWaitEvent(c->pipe_st[i], c->pipe_fork, 0);
+            if (e == cudaSuccess) {
+                const size_t npairs = (n + pf - 1) / pf, base = n / npairs, extra = n % npairs;  // balanced pairs
+                size_t f0 = 0;
+                cudaError_t el = cudaSuccess;
+                for (size_t k = 0; k < npairs && el == cudaSuccess; ++k) {
+                    const size_t m = base + (k < extra ? 1 : 0), off = f0 * c->g.frame_bytes;
+                    cudaStream_t sk = (k % S == 0) ? st : c->pipe_st[k % S - 1];
+                    el = decrypt ? vk::decrypt_tiled(c->g, c->plan, src + off, D + f0 * c->g.nD, B + off, m, dst + off, sk, &launches)
+                                 : vk::encrypt_tiled(c->g, c->plan, src + off, D + f0 * c->g.nD, B + off, m, dst + off, sk, &launches);
+                    f0 += m;
+                }
+                // join even after a failed launch: whatever was enqueued on the internal streams stays ordered before the
+                // caller's next operation
+                for (int i = 0; i + 1 < S; ++i) {
+                    cudaError_t ej = cudaEventRecord(c->pipe_join[i], c->pipe_st[i]);
+                    if (ej == cudaSuccess) ej = cudaStreamWaitEvent(st, c->pipe_join[i], 0);
+                    if (e == cudaSuccess) e = ej;
+                }
+                if (el != cudaSuccess) e = el;
+            }
+        } else {
+            e = decrypt ? vk::decrypt_tiled(c->g, c->plan, src, D, B, n, dst, st, &launches)
+                        : vk::encrypt_tiled(c->g, c->plan, src, D, B, n, dst, st, &launches);
+        }
     } else {
         uint8_t *out = dst;
         const size_t bytes = n * c->g.frame_bytes;
@@ -247,6 +292,14 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
         c->p = *p;
         c->g = vk::make_geom(p->width, p->height);
         c->batch = p->batch ? p->batch : 8;
+        c->pipe_streams = p->pipe_streams == 0 ? 2 : (int)(p->pipe_streams > (uint32_t)vcrypt_ctx::kPipeMax ? vcrypt_ctx::kPipeMax : p->pipe_streams);
+        {
+            // bytes of frames per launch pair, to the nearest frame.  Measured on B200 with two streams: 640x480 best at 30-40
+            // frames (28-37 MB), FHD at 5-6 (31-37 MB), 4K at 1 (25 MB): two pairs in flight keep their intermediates in L2
+            const size_t target = (size_t)34 << 20;
+            size_t pf = p->pipe_frames ? p->pipe_frames : (target + c->g.frame_bytes / 2) / c->g.frame_bytes;
+            c->pipe_frames = pf < 1 ? 1 : pf;
+        }
         c->simd = !(p->flags & VCRYPT_FLAG_HOST_SCALAR);
         c->isa = c->simd ? vh::best_isa() : 0;
         unsigned nt = p->host_threads ? p->host_threads : std::thread::hardware_concurrency();
@@ -293,6 +346,11 @@ extern "C" void vcrypt_destroy(vcrypt_ctx *c) {
     if (c->cuda) {
         cudaSetDevice(c->device);
         for (Slot &s : c->slots) free_slot(s);
+        for (int i = 0; i + 1 < vcrypt_ctx::kPipeMax; ++i) {
+            if (c->pipe_st[i]) { cudaStreamSynchronize(c->pipe_st[i]); cudaStreamDestroy(c->pipe_st[i]); }
+            if (c->pipe_join[i]) cudaEventDestroy(c->pipe_join[i]);
+        }
+        if (c->pipe_fork) cudaEventDestroy(c->pipe_fork);
         if (c->d_scratch) {
             cudaDeviceSynchronize();
             cudaFree(c->d_scratch);

@@ -1,6 +1,6 @@
 """Small timing probes of the individual device entry points (what profiles/ cites next to bench.py):
 
-  python -m paper_2505_07158_b200.probe kernels [--config C4] [--batch 8] [--batches 6]   encrypt / decrypt kernels, CUDA events
+  python -m paper_2505_07158_b200.probe kernels [--config C4] [--batch 8] [--batches 6] [--streams 1] | [--clip 96 --pipe-frames 0 --pipe-streams 0]   encrypt / decrypt kernels, CUDA events
   python -m paper_2505_07158_b200.probe derive  [--config C4] [--frames 8]                device hashing + worker systems, wall clock
   python -m paper_2505_07158_b200.probe stats   [--config C4] [--frames 32]               evaluation metrics, wall clock
 
@@ -29,9 +29,11 @@ def _hbm_peak() -> float:
         return 6650.0
 
 
-def kernels(cfg, batch: int, batches: int):
+def kernels(cfg, batch: int, batches: int, streams: int = 1, clip: int = 0, pipe_frames: int = 0, pipe_streams: int = 0):
     import torch
 
+    if clip:  # one call on a resident clip of `clip` frames: the library's own launch schedule (pipe_frames, pipe_streams)
+        batch, batches = clip, 1
     w, h, T = cfg.w, cfg.h, batch * batches
     g = torch.Generator(device="cuda")
     g.manual_seed(1)
@@ -39,21 +41,30 @@ def kernels(cfg, batch: int, batches: int):
     B = torch.randint(0, 256, (T, h, w, 3), dtype=torch.uint8, device="cuda", generator=g)
     D = torch.randint(-32768, 32767, (T, 3 * (h + w)), dtype=torch.int16, device="cuda", generator=g)
     E, P = torch.empty_like(F), torch.empty_like(F)
-    v = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, w, h)
-    st = torch.cuda.current_stream().cuda_stream
+    v = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, w, h, pipe_frames=pipe_frames, pipe_streams=pipe_streams)
+    # calls go round-robin over `streams` streams (independent batches: no ordering is needed between them);
+    # the timed region is bracketed on the current stream, which the side streams fork from and join into
+    cur = torch.cuda.current_stream()
+    side = [torch.cuda.Stream() for _ in range(streams)] if streams > 1 else [cur]
     alg = (9 * w * h + 6 * (w + h)) * T
     for name, fn, src, dst in (("encrypt", v.encrypt_device, F, E), ("decrypt", v.decrypt_device, E, P)):
         def run():
-            for b0 in range(0, T, batch):
-                fn(src[b0:b0 + batch], D[b0:b0 + batch], B[b0:b0 + batch], dst[b0:b0 + batch], st)
+            for k, b0 in enumerate(range(0, T, batch)):
+                fn(src[b0:b0 + batch], D[b0:b0 + batch], B[b0:b0 + batch], dst[b0:b0 + batch], side[k % len(side)].cuda_stream)
         for _ in range(3):
             run()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
+        e0.record(cur)
+        if streams > 1:
+            for s_ in side:
+                s_.wait_event(e0)
         for _ in range(10):
             run()
-        e1.record()
+        if streams > 1:
+            for s_ in side:
+                cur.wait_stream(s_)
+        e1.record(cur)
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / 10
         print(f"{cfg.name} {name}: {ms * 1e3 / T:.3f} us/frame, {alg / ms / 1e6:.0f} GB/s algorithmic, {alg / ms / 1e6 / _hbm_peak():.3f} of the HBM copy rate")
@@ -108,10 +119,14 @@ def main():
     ap.add_argument("--batch", type=int, default=8)
     ap.add_argument("--batches", type=int, default=6)
     ap.add_argument("--frames", type=int, default=0)
+    ap.add_argument("--streams", type=int, default=1, help="kernels: streams the calls go round-robin over")
+    ap.add_argument("--clip", type=int, default=0, help="kernels: one call on a resident clip of this many frames")
+    ap.add_argument("--pipe-frames", type=int, default=0, help="kernels: vcrypt_params.pipe_frames (0: library default)")
+    ap.add_argument("--pipe-streams", type=int, default=0, help="kernels: vcrypt_params.pipe_streams (0: library default, 1: off)")
     a = ap.parse_args()
     cfg = synth.CONFIGS[a.config]
     if a.what == "kernels":
-        kernels(cfg, a.batch, a.batches)
+        kernels(cfg, a.batch, a.batches, a.streams, a.clip, a.pipe_frames, a.pipe_streams)
     elif a.what == "derive":
         derive(cfg, a.frames or 8)
     else:

@@ -156,10 +156,56 @@ def test_many_frames_per_call_split_into_l2_sized_launches(torch_cuda, vb, orc):
     """More frames than one L2-resident launch holds: the call splits, results unchanged."""
     w, h, nf = 640, 480, 120  # 110.6 MB of frames: two launch pairs (113 + 7 frames)
     F, D, B = rnd_case(w, h, nf, seed=21)
-    v = gpu_ctx(vb, w, h)
+    v = gpu_ctx(vb, w, h, pipe_streams=1)  # every launch on the caller's stream
     E = run_device(torch_cuda, v, F, D, B)
     assert v.launch_count()[0] == 4
     for k in (0, 1, 37, 112, 113, 114, 119):
+        assert np.array_equal(E[k], orc.confuse_xor(F[k], D[k], B[k])), k
+    assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
+
+
+@pytest.mark.parametrize("w,h,nf,pf,ps", [(64, 48, 11, 2, 2), (80, 32, 13, 3, 3), (256, 256, 9, 1, 4), (112, 20, 8, 4, 2),
+                                          (64, 16, 7, 3, 9)])
+def test_resident_clip_schedule_over_streams(torch_cuda, vb, orc, w, h, nf, pf, ps):
+    """A call that brings >= 2 * pipe_frames frames alternates its launch pairs over pipe_streams streams (forked from and
+    joined into the caller's stream): balanced pairs with a ragged count, every frame bit-exact, both directions, in place
+    too, and ordered with respect to the caller's stream (the very next operation on it reads the result)."""
+    F, D, B = rnd_case(w, h, nf, seed=31 + nf)
+    want = oracle_frames(orc, F, D, B)
+    v = gpu_ctx(vb, w, h, pipe_frames=pf, pipe_streams=ps)
+    E = run_device(torch_cuda, v, F, D, B)
+    npairs = -(-nf // pf)
+    assert v.launch_count()[0] == 2 * npairs
+    assert np.array_equal(E, want)
+    assert np.array_equal(run_device(torch_cuda, v, F, D, B, inplace=True), want)
+    assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
+    # stream order: on a side stream, the copy enqueued right after the call must see the finished ciphertext
+    torch = torch_cuda
+    dF, dB = torch.from_numpy(F).cuda(), torch.from_numpy(B).cuda()
+    dD = torch.from_numpy(D.view(np.int16)).cuda()
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        for _ in range(3):
+            dE = torch.zeros_like(dF)
+            v.encrypt_device(dF, dD, dB, dE, side.cuda_stream)
+            host = torch.empty(dE.shape, dtype=dE.dtype).pin_memory()
+            host.copy_(dE, non_blocking=True)
+            side.synchronize()
+            assert np.array_equal(host.numpy(), want)
+    # a single-stream context gives the same bytes
+    v1 = gpu_ctx(vb, w, h, pipe_streams=1)
+    assert np.array_equal(run_device(torch_cuda, v1, F, D, B), want)
+
+
+def test_resident_clip_schedule_defaults(torch_cuda, vb, orc):
+    """Default pipe_frames (about 34 MB of frames per launch pair): 640 x 480 -> 39 frames, so 120 frames = 4 pairs of 30."""
+    w, h, nf = 640, 480, 120
+    F, D, B = rnd_case(w, h, nf, seed=22)
+    v = gpu_ctx(vb, w, h)
+    E = run_device(torch_cuda, v, F, D, B)
+    assert v.launch_count()[0] == 8
+    for k in (0, 29, 30, 59, 60, 89, 90, 119):
         assert np.array_equal(E[k], orc.confuse_xor(F[k], D[k], B[k])), k
     assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
 
