@@ -36,10 +36,11 @@ from paper_2505_07158_b200 import parallel, synth  # noqa: E402
 METRIC = "FHD frames/s encrypted"
 UNIT = "frames/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum of the two kernels of one encrypt call (8 FHD frames; 2 4K frames per
-# launch pair), from the ncu --set full capture summarised in profiles/r1f_ncu_full_summary.csv
-NCU_TRAFFIC_PER_CALL = {"C4": 142.0e6}  # bytes; part of the 149.4 MB of a call is output still dirty in L2 when it ends
-NCU_COL_SHARE = 0.585
+# dram__bytes_read.sum + dram__bytes_write.sum of the two kernels of one launch pair (6 FHD frames: row pass 37.2 + 4.9 MB,
+# column pass 39.8 + 5.8 MB), from the ncu --set full capture summarised in profiles/r1m_ncu_full_summary.csv; below the
+# 112.1 MB of algorithmic bytes of a pair because most of its output is still dirty in L2 when the kernel ends
+NCU_TRAFFIC_PER_CALL = {"C4": 87.7e6}
+NCU_COL_SHARE = 0.54  # column pass's share of a launch pair's serialised time in the same capture (21.9 of 40.4 us)
 
 
 def hbm_peak():

@@ -143,7 +143,11 @@ int vcrypt_host_threads(const vcrypt_ctx *ctx);
  * hrot = row i0 of channel c rotated by d_h(i0,c) mod 8w bit positions toward higher columns, LSB first.
  * d_frames, d_B, d_cipher: device, n x H x W x 3; d_D: device, n x 3(H+W) uint16.  d_cipher may equal
  * d_frames (in place); it must not partially overlap.  cuda_stream: a cudaStream_t (NULL = default stream).
- * Asynchronous: returns after enqueueing; launch errors are reported, execution errors surface on sync. */
+ * Asynchronous: returns after enqueueing; launch errors are reported, execution errors surface on sync.
+ * Stream order: everything the call enqueues is ordered after the work already in cuda_stream and before whatever
+ * the caller enqueues there next -- also when a call on a long resident clip (n >= 2 x pipe_frames) spreads its
+ * launch pairs over internal streams (vcrypt_params.pipe_frames / pipe_streams): those fork from cuda_stream at the
+ * start of the call and join it at the end (legal under stream capture). */
 int vcrypt_encrypt_device(vcrypt_ctx *ctx, const void *d_frames, const void *d_D, const void *d_B, size_t n,
                           void *d_cipher, void *cuda_stream);
 
