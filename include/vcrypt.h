@@ -81,7 +81,7 @@ typedef struct vcrypt_params {
                                hashes (the last ones; the host threads hash the others at the same time);
                                0 or values above n -> all n.  Does not affect results                          */
     uint32_t pipe_frames;   /* vcrypt_{en,de}crypt_device on a resident clip: frames per launch pair when a call brings
-                               at least 2 x pipe_frames frames; such a call alternates its launch pairs over
+                               at least 4 x pipe_frames frames; such a call alternates its launch pairs over
                                `pipe_streams` streams (the caller's + internal ones forked from and joined into it),
                                so that one pair's column pass overlaps the next pair's row pass.  0 -> from the frame
                                size (about 37 MB of frames per pair).  Does not affect results                     */
@@ -145,7 +145,7 @@ int vcrypt_host_threads(const vcrypt_ctx *ctx);
  * d_frames (in place); it must not partially overlap.  cuda_stream: a cudaStream_t (NULL = default stream).
  * Asynchronous: returns after enqueueing; launch errors are reported, execution errors surface on sync.
  * Stream order: everything the call enqueues is ordered after the work already in cuda_stream and before whatever
- * the caller enqueues there next -- also when a call on a long resident clip (n >= 2 x pipe_frames) spreads its
+ * the caller enqueues there next -- also when a call on a long resident clip (n >= 4 x pipe_frames) spreads its
  * launch pairs over internal streams (vcrypt_params.pipe_frames / pipe_streams): those fork from cuda_stream at the
  * start of the call and join it at the end (legal under stream capture). */
 int vcrypt_encrypt_device(vcrypt_ctx *ctx, const void *d_frames, const void *d_D, const void *d_B, size_t n,

@@ -206,7 +206,7 @@ int launch_cipher(vcrypt_ctx *c, bool decrypt, const uint8_t *src, const uint16_
     const bool aligned = ((((uintptr_t)src) | ((uintptr_t)dst) | ((uintptr_t)B)) & 15u) == 0;
     if (c->plan.tiled && aligned && !(c->p.flags & VCRYPT_FLAG_FORCE_GENERIC)) {
         const size_t pf = c->pipe_frames;
-        if (c->pipe_streams >= 2 && n >= 2 * pf) {
+        if (c->pipe_streams >= 2 && n >= 4 * pf) {  // fewer pairs never reach a steady state: the fork / join costs more than it hides
             // Resident clip.  The two passes of a launch pair stress different parts of the memory system (the row pass
             // reads DRAM and fills L2, the column pass's CTAs first pull their strips out of L2 and then stream DRAM), and
             // inside one stream a pass only starts when its predecessor has drained.  Frames are independent, so the

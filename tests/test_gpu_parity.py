@@ -164,10 +164,10 @@ def test_many_frames_per_call_split_into_l2_sized_launches(torch_cuda, vb, orc):
     assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
 
 
-@pytest.mark.parametrize("w,h,nf,pf,ps", [(64, 48, 11, 2, 2), (80, 32, 13, 3, 3), (256, 256, 9, 1, 4), (112, 20, 8, 4, 2),
-                                          (64, 16, 7, 3, 9)])
+@pytest.mark.parametrize("w,h,nf,pf,ps", [(64, 48, 11, 2, 2), (80, 32, 13, 3, 3), (256, 256, 9, 1, 4), (112, 20, 17, 4, 2),
+                                          (64, 16, 14, 3, 9)])
 def test_resident_clip_schedule_over_streams(torch_cuda, vb, orc, w, h, nf, pf, ps):
-    """A call that brings >= 2 * pipe_frames frames alternates its launch pairs over pipe_streams streams (forked from and
+    """A call that brings >= 4 * pipe_frames frames alternates its launch pairs over pipe_streams streams (forked from and
     joined into the caller's stream): balanced pairs with a ragged count, every frame bit-exact, both directions, in place
     too, and ordered with respect to the caller's stream (the very next operation on it reads the result)."""
     F, D, B = rnd_case(w, h, nf, seed=31 + nf)
@@ -199,15 +199,18 @@ def test_resident_clip_schedule_over_streams(torch_cuda, vb, orc, w, h, nf, pf, 
 
 
 def test_resident_clip_schedule_defaults(torch_cuda, vb, orc):
-    """Default pipe_frames (about 34 MB of frames per launch pair): 640 x 480 -> 39 frames, so 120 frames = 4 pairs of 30."""
-    w, h, nf = 640, 480, 120
+    """Default pipe_frames (about 34 MB of frames per launch pair): 640 x 480 -> 39 frames; 160 frames >= 4 x 39 = 5 pairs of
+    32, while 120 frames stay on the caller's stream (test_many_frames_per_call... covers the split by L2 budget)."""
+    w, h, nf = 640, 480, 160
     F, D, B = rnd_case(w, h, nf, seed=22)
     v = gpu_ctx(vb, w, h)
     E = run_device(torch_cuda, v, F, D, B)
-    assert v.launch_count()[0] == 8
-    for k in (0, 29, 30, 59, 60, 89, 90, 119):
+    assert v.launch_count()[0] == 10
+    for k in (0, 31, 32, 63, 64, 95, 96, 127, 128, 159):
         assert np.array_equal(E[k], orc.confuse_xor(F[k], D[k], B[k])), k
     assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
+    E2 = run_device(torch_cuda, v, F[:120], D[:120], B[:120])
+    assert v.launch_count()[0] == 4 and np.array_equal(E2, E[:120])
 
 
 def test_device_call_argument_errors(torch_cuda, vb):
