@@ -198,6 +198,32 @@ def test_resident_clip_schedule_over_streams(torch_cuda, vb, orc, w, h, nf, pf, 
     assert np.array_equal(run_device(torch_cuda, v1, F, D, B), want)
 
 
+def test_resident_clip_schedule_under_stream_capture(torch_cuda, vb, orc):
+    """The fork / join over the internal stream is a legal capture pattern: the call is recorded into a CUDA graph and the
+    replays (on new inputs in the same buffers) are bit-exact."""
+    torch = torch_cuda
+    w, h, nf = 64, 48, 12
+    v = gpu_ctx(vb, w, h, pipe_frames=3, pipe_streams=2)
+    F, D, B = rnd_case(w, h, nf, seed=77)
+    dF, dB = torch.from_numpy(F).cuda(), torch.from_numpy(B).cuda()
+    dD = torch.from_numpy(D.view(np.int16)).cuda()
+    dE = torch.zeros_like(dF)
+    v.encrypt_device(dF, dD, dB, dE)  # warm-up outside the capture: creates the internal stream and events
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        v.encrypt_device(dF, dD, dB, dE, torch.cuda.current_stream().cuda_stream)
+    for seed in (78, 79):
+        F2, D2, B2 = rnd_case(w, h, nf, seed=seed)
+        dF.copy_(torch.from_numpy(F2))
+        dB.copy_(torch.from_numpy(B2))
+        dD.copy_(torch.from_numpy(D2.view(np.int16)))
+        dE.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(dE.cpu().numpy(), oracle_frames(orc, F2, D2, B2)), seed
+
+
 def test_resident_clip_schedule_defaults(torch_cuda, vb, orc):
     """Default pipe_frames (about 34 MB of frames per launch pair): 640 x 480 -> 39 frames; 160 frames >= 4 x 39 = 5 pairs of
     32, while 120 frames stay on the caller's stream (test_many_frames_per_call... covers the split by L2 budget)."""
