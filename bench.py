@@ -36,11 +36,11 @@ from paper_2505_07158_b200 import parallel, synth  # noqa: E402
 METRIC = "FHD frames/s encrypted"
 UNIT = "frames/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum of the two kernels of one launch pair (6 FHD frames: row pass 37.2 + 4.9 MB,
-# column pass 39.8 + 5.8 MB), from the ncu --set full capture summarised in profiles/r1m_ncu_full_summary.csv; below the
-# 112.1 MB of algorithmic bytes of a pair because most of its output is still dirty in L2 when the kernel ends
-NCU_TRAFFIC_PER_CALL = {"C4": 87.7e6}
-NCU_COL_SHARE = 0.54  # column pass's share of a launch pair's serialised time in the same capture (21.9 of 40.4 us)
+# dram__bytes_read.sum + dram__bytes_write.sum of the two kernels of one launch pair (5 FHD frames: row pass 30.9 + 2.9 MB,
+# column pass 27.0 + 3.2 MB), from the ncu --set full capture summarised in profiles/r1n_ncu_full_summary.csv; below the
+# 93.4 MB of algorithmic bytes of a pair because most of its output is still dirty in L2 when the kernel ends
+NCU_TRAFFIC_PER_CALL = {"C4": 64.0e6}
+NCU_COL_SHARE = 0.544  # column pass's share of a launch pair's serialised time in the same capture (19.6 of 36.1 us)
 
 
 def hbm_peak():
@@ -134,7 +134,7 @@ def run_reference(args, cfg):
 def workload_name(cfg):
     return (f"{cfg.name}: {cfg.w}x{cfg.h}x3 uint8 synthetic video (moving gradient + blocks + noise), {cfg.frames} frames, "
             f"end-to-end leg in batches of {cfg.batch} per launch pair over e2e.n_streams streams; kernel-only leg = one call on the "
-            f"resident clip (launch pairs of about 34 MB of frames over 2 streams), "
+            f"resident clip (launch pairs of about 31 MB of frames over 2 streams), "
             f"key = 4 doubles, n_workers = {synth.N_WORKERS}")
 
 
@@ -214,7 +214,7 @@ def main():
     stream = torch.cuda.current_stream().cuda_stream
 
     def kernel_step():
-        # one call on the resident clip: the library cuts it into launch pairs (row pass + column pass) of about 34 MB of
+        # one call on the resident clip: the library cuts it into launch pairs (row pass + column pass) of about 31 MB of
         # frames and alternates them over two streams forked from / joined into `stream` (vcrypt_params.pipe_*)
         kctx.encrypt_device(d_F, d_D, d_B, d_E, stream)
         return kctx.launch_count()[0]

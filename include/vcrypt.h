@@ -84,7 +84,7 @@ typedef struct vcrypt_params {
                                at least 4 x pipe_frames frames; such a call alternates its launch pairs over
                                `pipe_streams` streams (the caller's + internal ones forked from and joined into it),
                                so that one pair's column pass overlaps the next pair's row pass.  0 -> from the frame
-                               size (about 37 MB of frames per pair).  Does not affect results                     */
+                               size (about 31 MB of frames per pair when encrypting, 37 MB when decrypting).  Does not affect results                     */
     uint32_t pipe_streams;  /* 0 -> 2; 1 -> off (every launch on the caller's stream); at most 4                    */
 } vcrypt_params;
 

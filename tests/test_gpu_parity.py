@@ -225,8 +225,8 @@ def test_resident_clip_schedule_under_stream_capture(torch_cuda, vb, orc):
 
 
 def test_resident_clip_schedule_defaults(torch_cuda, vb, orc):
-    """Default pipe_frames (about 34 MB of frames per launch pair): 640 x 480 -> 39 frames; 160 frames >= 4 x 39 = 5 pairs of
-    32, while 120 frames stay on the caller's stream (test_many_frames_per_call... covers the split by L2 budget)."""
+    """Default pipe_frames (about 31 MB of frames per launch pair when encrypting): 640 x 480 -> 35 frames; 160 frames >= 4 x 35
+    = 5 pairs of 32, while 120 frames stay on the caller's stream (test_many_frames_per_call... covers the split by L2 budget)."""
     w, h, nf = 640, 480, 160
     F, D, B = rnd_case(w, h, nf, seed=22)
     v = gpu_ctx(vb, w, h)
