@@ -215,6 +215,17 @@ int vcrypt_local_entropy_device(vcrypt_ctx *ctx, const void *d_frames, size_t n,
  * Allocates and frees about 3.6 GB of device memory.  VCRYPT_E_ARG for a bad `which`, frames = 0 or reps < 1. */
 int vcrypt_memory_probe(vcrypt_ctx *ctx, int which, size_t frames, int reps, double *us_per_rep);
 
+/* Distributed-shared-memory exchange probe (design hook): as many thread-block clusters of
+ * `cluster_size` CTAs (1 .. 16; sizes above 8 are non-portable) as are resident at once, every CTA owning
+ * `bytes_per_cta` bytes of shared memory (a multiple of 16 x cluster_size; twice that + 64 must fit the per-CTA
+ * limit); per round every CTA sends bytes_per_cta / cluster_size bytes to each CTA of its cluster -- one all-to-all
+ * of cluster_size x bytes_per_cta bytes per cluster -- with 16-byte st.shared::cluster stores (mode 0) or
+ * cp.async.bulk shared -> peer shared with mbarrier completion (mode 1).  Returns the mean time of one round in
+ * microseconds (CUDA events, `rounds` rounds in one launch, cluster barrier per round) and the number of resident
+ * clusters.  VCRYPT_E_ARG for sizes that do not fit. */
+int vcrypt_dsmem_probe(vcrypt_ctx *ctx, int cluster_size, size_t bytes_per_cta, int mode, int rounds, double *us_per_round,
+                       int *resident_clusters);
+
 #ifdef __cplusplus
 }
 #endif

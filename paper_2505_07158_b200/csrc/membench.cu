@@ -9,6 +9,10 @@
 //   probe 2  column strips              : read B and write O in 64-byte-wide column strips of the h x 3w matrix
 //                                          (the DRAM side of the column pass: row-strided 64-byte accesses)
 // Buffers rotate through > 1 GB so that nothing but T is L2-resident between repetitions.
+//
+// dsmem_probe (vcrypt_dsmem_probe) answers a design question instead: how fast can the CTAs of a
+// thread-block cluster exchange an all-to-all through distributed shared memory -- the alternative to passing the
+// intermediate between row owners and column owners through L2.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -103,6 +107,129 @@ cudaError_t memory_probe(const Geom &g, int which, size_t frames, int reps, cuda
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
     cudaFree(A); cudaFree(Bb); cudaFree(O); cudaFree(T);
+    return e;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Distributed-shared-memory exchange: every CTA of a cluster owns `own` bytes of shared memory and, per round, sends
+// own / CS bytes to each of the CS CTAs of its cluster (itself included), i.e. the cluster performs one all-to-all of
+// CS * own bytes.  mode 0: 16-byte st.shared::cluster stores by the threads; mode 1: one cp.async.bulk shared::cta ->
+// shared::cluster per peer with completion on the peer's mbarrier.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t pb_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t pb_mapa(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void pb_cluster_sync() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(512, 1) probe_dsmem(uint32_t own, uint32_t rounds, uint32_t *sink) {
+    extern __shared__ __align__(128) uint8_t PS[];
+    uint32_t CS, rank;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(CS));
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    uint8_t *strip = PS, *src = PS + own;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(PS + 2u * own);
+    const uint32_t piece = own / CS;
+    for (uint32_t i = threadIdx.x; i < own / 4u; i += blockDim.x) reinterpret_cast<uint32_t *>(src)[i] = i * 2654435761u + rank;
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(pb_smem_u32(bar)));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    pb_cluster_sync();
+    for (uint32_t r = 0; r < rounds; ++r) {
+        if (MODE == 0) {
+            for (uint32_t i = threadIdx.x; i < own / 16u; i += blockDim.x) {
+                const uint32_t byte = i * 16u, p = byte / piece, off = byte - p * piece;
+                const uint4 v = *reinterpret_cast<const uint4 *>(src + byte);
+                const uint32_t dst = pb_mapa(pb_smem_u32(strip + rank * piece + off), p);
+                asm volatile("st.shared::cluster.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(dst), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+            }
+            pb_cluster_sync();
+        } else {
+            if (threadIdx.x == 0)
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(pb_smem_u32(bar)), "r"(piece * CS) : "memory");
+            pb_cluster_sync();  // every barrier of the cluster is armed
+            if (threadIdx.x < CS) {
+                const uint32_t p = threadIdx.x;
+                const uint32_t dst = pb_mapa(pb_smem_u32(strip + rank * piece), p), rbar = pb_mapa(pb_smem_u32(bar), p);
+                asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                             "r"(pb_smem_u32(src + p * piece)), "r"(piece), "r"(rbar)
+                             : "memory");
+            }
+            uint32_t ok = 0, spin = 0;
+            while (!ok) {
+                asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                             : "=r"(ok)
+                             : "r"(pb_smem_u32(bar)), "r"(r & 1u)
+                             : "memory");
+                if (++spin > (1u << 24)) __trap();  // a copy that never lands must trap, not hang the GPU
+            }
+            pb_cluster_sync();
+        }
+    }
+    if (threadIdx.x == 0) {
+        uint32_t acc = 0;
+        for (uint32_t i = 0; i < own / 4u; i += 97u) acc += reinterpret_cast<uint32_t *>(strip)[i];
+        sink[blockIdx.x] = acc;
+    }
+}
+
+cudaError_t dsmem_probe(int cluster_size, size_t own_bytes, int mode, int rounds, double *us_per_round, int *max_active_clusters,
+                        int *clusters_launched) {
+    if (cluster_size < 1 || cluster_size > 16 || (mode != 0 && mode != 1) || rounds < 1) return cudaErrorInvalidValue;
+    if (own_bytes < 16u * (size_t)cluster_size || own_bytes % (16u * (size_t)cluster_size) != 0) return cudaErrorInvalidValue;
+    int dev = 0, sms = 0, smem_optin = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (!e) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (!e) e = cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e) return e;
+    const size_t smem = 2 * own_bytes + 64;
+    if (smem > (size_t)smem_optin) return cudaErrorInvalidValue;
+    void (*k)(uint32_t, uint32_t, uint32_t *) = mode == 0 ? probe_dsmem<0> : probe_dsmem<1>;
+    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (!e) e = cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e) return e;
+    cudaLaunchConfig_t cfg{};
+    cfg.blockDim = dim3(512);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)cluster_size;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cfg.gridDim = dim3((unsigned)cluster_size);
+    int maxc = 0;
+    e = cudaOccupancyMaxActiveClusters(&maxc, k, &cfg);
+    if (e) return e;
+    if (max_active_clusters) *max_active_clusters = maxc;
+    if (maxc < 1) return cudaErrorInvalidValue;
+    if (clusters_launched) *clusters_launched = maxc;
+    cfg.gridDim = dim3((unsigned)(cluster_size * maxc));  // one resident wave
+    uint32_t *sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    e = cudaMalloc(&sink, sizeof(uint32_t) * cluster_size * maxc);
+    if (!e) e = cudaEventCreate(&e0);
+    if (!e) e = cudaEventCreate(&e1);
+    if (!e) e = cudaLaunchKernelEx(&cfg, k, (uint32_t)own_bytes, (uint32_t)rounds, sink);  // warm-up
+    if (!e) e = cudaEventRecord(e0, 0);
+    if (!e) e = cudaLaunchKernelEx(&cfg, k, (uint32_t)own_bytes, (uint32_t)rounds, sink);
+    if (!e) e = cudaEventRecord(e1, 0);
+    if (!e) e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (!e) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (!e && us_per_round) *us_per_round = 1e3 * (double)ms / rounds;
+    cudaDeviceSynchronize();
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(sink);
     return e;
 }
 

@@ -737,6 +737,21 @@ extern "C" int vcrypt_memory_probe(vcrypt_ctx *c, int which, size_t frames, int 
     });
 }
 
+extern "C" int vcrypt_dsmem_probe(vcrypt_ctx *c, int cluster_size, size_t bytes_per_cta, int mode, int rounds, double *us_per_round,
+                                  int *resident_clusters) {
+    return guarded([&]() -> int {
+        if (!c || !us_per_round) return VCRYPT_E_ARG;
+        if (!c->cuda) return VCRYPT_E_CUDA;
+        VC_CUDA(c, cudaSetDevice(c->device));
+        int maxc = 0, launched = 0;
+        const cudaError_t e = vk::dsmem_probe(cluster_size, bytes_per_cta, mode, rounds, us_per_round, &maxc, &launched);
+        if (resident_clusters) *resident_clusters = launched;
+        if (e == cudaErrorInvalidValue) { cudaGetLastError(); return VCRYPT_E_ARG; }
+        if (e != cudaSuccess) return cuda_fail(c, e, "dsmem probe");
+        return VCRYPT_OK;
+    });
+}
+
 // =====================================================================================================
 // host-buffer pipeline: Algorithm 1's loop over frames, batched and overlapped
 // =====================================================================================================

@@ -3,6 +3,7 @@
   python -m paper_2505_07158_b200.probe kernels [--config C4] [--batch 8] [--batches 6] [--streams 1] | [--clip 96 --pipe-frames 0 --pipe-streams 0]   encrypt / decrypt kernels, CUDA events
   python -m paper_2505_07158_b200.probe derive  [--config C4] [--frames 8]                device hashing + worker systems, wall clock
   python -m paper_2505_07158_b200.probe stats   [--config C4] [--frames 32]               evaluation metrics, wall clock
+  python -m paper_2505_07158_b200.probe dsmem                                             all-to-all through distributed shared memory
 
 Inputs are random device tensors (the kernels' time does not depend on the values); results are only timed here --
 parity lives in tests/.  Needs a CUDA device.
@@ -112,9 +113,26 @@ def stats(cfg, frames: int):
         print(f"{cfg.name} {name}: {dt * 1e3:.3f} ms per call of {frames} frames (device + host finish){extra}")
 
 
+def dsmem(cfg):
+    """What an all-to-all between the CTAs of a cluster costs through distributed shared memory."""
+    v = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    for cs in (2, 4, 8, 16):
+        for kb in (64, 96, 110):
+            own = kb * 1024 // (16 * cs) * (16 * cs)
+            for mode, name in ((0, "st.shared::cluster.v4"), (1, "cp.async.bulk to peer")):
+                try:
+                    us, nc = v.dsmem_probe(cs, own, mode, 20)
+                except vb.VcryptError as e:
+                    print(f"cluster {cs:2d} x {kb:3d} KB {name}: {e}")
+                    continue
+                tot = own * cs * nc
+                print(f"cluster {cs:2d} x {kb:3d} KB per CTA, {nc:2d} resident clusters ({cs * nc:3d} SMs), {name:22s}: "
+                      f"{us:6.2f} us per all-to-all, {tot / us / 1e6:5.2f} TB/s chip-wide, {own / (us * 1e-6) / 1.965e9:5.1f} B/clk/SM at 1965 MHz")
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
-    ap.add_argument("what", choices=["kernels", "derive", "stats"])
+    ap.add_argument("what", choices=["kernels", "derive", "stats", "dsmem"])
     ap.add_argument("--config", default="C4", choices=sorted(synth.CONFIGS))
     ap.add_argument("--batch", type=int, default=8)
     ap.add_argument("--batches", type=int, default=6)
@@ -127,6 +145,8 @@ def main():
     cfg = synth.CONFIGS[a.config]
     if a.what == "kernels":
         kernels(cfg, a.batch, a.batches, a.streams, a.clip, a.pipe_frames, a.pipe_streams)
+    elif a.what == "dsmem":
+        dsmem(cfg)
     elif a.what == "derive":
         derive(cfg, a.frames or 8)
     else:

@@ -450,6 +450,17 @@ def test_memory_probe_hook(vb):
     assert v.L.vcrypt_memory_probe(v._p, 0, 1, 1, None) == vb.E_ARG
 
 
+def test_dsmem_probe_hook(vb):
+    """Design hook: an all-to-all between the CTAs of a cluster through distributed shared memory runs and is timed."""
+    v = gpu_ctx(vb, 256, 256)
+    for cs, own, mode in ((2, 32 * 1024, 0), (8, 64 * 1024, 1), (16, 64 * 1024, 0)):
+        us, nc = v.dsmem_probe(cs, own, mode, 4)
+        assert us > 0 and nc >= 1
+    for cs, own, mode in ((0, 65536, 0), (17, 65536, 0), (8, 65536, 2), (8, 1000, 0), (8, 200 * 1024, 0)):
+        with pytest.raises(vb.VcryptError):
+            v.dsmem_probe(cs, own, mode, 4)
+
+
 def test_failed_call_leaves_chain_untouched(vb):
     v = gpu_ctx(vb, 64, 48)
     s0 = v.get_state()
