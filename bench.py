@@ -232,8 +232,16 @@ def main():
         torch.cuda.synchronize()
 
     # ---- kernel-only: CUDA events on the launching stream -----------------------------------------------
-    for _ in range(W):
+    # W untimed steps; a kernel-only step lasts about a millisecond, so the warm-up is also held for at least 50 ms of GPU
+    # work: the timed steps must not see the clock ramp of a GPU that idled during the host-side set-up.  (Measured: 3 steps
+    # or 50 ms of warm-up -> 0.600 - 0.604 of the copy rate; 250 ms of warm-up -> 0.594 with sw_power_cap reported: the
+    # timed region of 10 steps is 14 ms, a burst like the copy the peak was measured with.)
+    warm_steps, t_warm = 0, time.perf_counter()
+    while warm_steps < W or (time.perf_counter() - t_warm < 0.05 and warm_steps < 2000):
         kernel_step()
+        warm_steps += 1
+        if warm_steps >= W:
+            torch.cuda.synchronize()
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
@@ -380,7 +388,7 @@ def main():
         "dtype": "u8", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "frames_per_step": T, "ms_per_frame_kernel": kern_ms_total / K / T,
                    "l2": f"inputs larger than L2: {3 * fb * T / 1e6:.0f} MB streamed per step, no flush needed",
-                   "host_threads": threads, "host_cores": ncores, "describe": vb.describe()},
+                   "host_threads": threads, "host_cores": ncores, "warmup_steps_run": warm_steps, "describe": vb.describe()},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": T * ((fb + 64 * synth.N_WORKERS) if args.derive == "device" else (2 * fb + 2 * nD)),
                 "d2h_bytes_per_step": T * fb,
                 "ms_per_frame": 1e3 * e2e_total / (K * T), "ms_per_step_median": 1e3 * statistics.median(e2e_s),
