@@ -31,7 +31,9 @@
 // The intermediate between the passes lives in the output buffer (every CTA of either pass reads all
 // of its rows / its whole strip before it writes them), and launches are sized so that it stays
 // resident in the 126 MB L2: DRAM traffic stays at the algorithmic read F_o + read B + write F_e.
-// The kernels of one call are chained with programmatic dependent launch (griddepcontrol).
+// The kernels of one call are chained with programmatic dependent launch (griddepcontrol); a call on a long resident clip
+// is cut into launch pairs (row pass + column pass) that alternate over two streams, so that one pair's column pass
+// overlaps the next pair's row pass (vcrypt.cpp: launch_cipher).
 //
 // A one-thread-per-output-byte gather kernel covers every shape the tiled passes do not
 // (w % 16 != 0, w < 64, h % 4 != 0, h < 16, or a strip / row block too large for shared memory).
