@@ -253,6 +253,36 @@ def test_device_call_argument_errors(torch_cuda, vb):
     assert L.vcrypt_encrypt_device(v._p, dF.data_ptr(), dD.data_ptr(), dB.data_ptr(), 0, dF.data_ptr(), st) == vb.OK
 
 
+@pytest.mark.parametrize("cfgname,nf,pairs_enc,pairs_dec", [("C4", 30, 6, 5), ("C5", 8, 8, 4)])
+def test_full_size_resident_clip_as_bench_times_it(torch_cuda, vb, orc, cfgname, nf, pairs_enc, pairs_dec):
+    """The launch configuration bench.py's kernel leg times -- ONE *_device call on a resident clip with the default schedule
+    (FHD: launch pairs of 5 frames when encrypting, 6 when decrypting; 4K: 1 and 2) -- at full frame size, sampled frames
+    against the oracle, every frame through the inverse."""
+    torch = torch_cuda
+    cfg = synth.CONFIGS[cfgname]
+    w, h = cfg.w, cfg.h
+    F, D, B = rnd_case(w, h, nf, seed=41)
+    v = gpu_ctx(vb, w, h)
+    dF, dB = torch.from_numpy(F).cuda(), torch.from_numpy(B).cuda()
+    dD = torch.from_numpy(D.view(np.int16)).cuda()
+    dE = torch.empty_like(dF)
+    v.encrypt_device(dF, dD, dB, dE)
+    torch.cuda.synchronize()
+    assert v.launch_count()[0] == 2 * pairs_enc
+    for k in sorted({0, nf // 2 - 1, nf // 2, nf - 1}):
+        assert np.array_equal(dE[k].cpu().numpy(), orc.confuse_xor(F[k], D[k], B[k])), k
+    dP = torch.empty_like(dF)
+    v.decrypt_device(dE, dD, dB, dP)
+    torch.cuda.synchronize()
+    assert v.launch_count()[0] == 2 * pairs_dec
+    assert bool(torch.equal(dP, dF))
+    # the same call repeated in place gives the same bytes (no dependence on what the streams did before)
+    dG = dF.clone()
+    v.encrypt_device(dG, dD, dB, dG)
+    torch.cuda.synchronize()
+    assert bool(torch.equal(dG, dE))
+
+
 # ------------------------------------------------------------------------------------------------------
 # whole path
 # ------------------------------------------------------------------------------------------------------
