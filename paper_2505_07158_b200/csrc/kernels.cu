@@ -869,6 +869,16 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
             p.col_ctas_per_sm = ctas;
             p.strips_per_frame = (int)((g.row_bytes + X - 1) / X);
             p.smem_cole = cole_smem_bytes(g, X);
+            // Encrypt direction: when three CTAs per SM would need the largest shared-memory carve-out (more than 196 KB with the
+            // 1 KB the system reserves per CTA), ask for so much that only TWO fit.  Measured on B200 under the two-stream schedule,
+            // ns per frame row at w = 1920: strips up to h = 1008 (three CTAs inside 196 KB) 4.13 - 4.15, h = 1024 .. 1184 (three CTAs,
+            // 228 KB) 4.37 - 4.42, h >= 1200 (two CTAs) 4.12; FHD with the larger request 4.74 -> 4.49 us per frame.  The decrypt
+            // direction, whose CTAs also convert their strip in shared memory, is faster with three (5.56 against 5.71).
+            p.smem_cole_enc = p.smem_cole;
+            if (ctas == 3 && 3 * (p.smem_cole + 1024) > (size_t)196 * 1024) {
+                const size_t two_only = ((size_t)smem_sm / 3 - 1024 + 255) / 128 * 128;  // 3 x (this + 1 KB) > shared memory of an SM
+                if (two_only > p.smem_cole && two_only <= (size_t)smem_optin) p.smem_cole_enc = two_only;
+            }
             uint32_t br = 1;
             for (uint32_t d = 1; d <= 256 && d <= g.h; ++d)
                 if (g.h % d == 0) br = d;
@@ -890,11 +900,11 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
             const size_t l2_budget = (size_t)100 << 20;
             p.max_frames_per_launch = l2_budget / g.frame_bytes ? l2_budget / g.frame_bytes : 1;
             if (ctas == 3) {
-                if (X == 64) { e = col_set_attr<64, 256, 3>(p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3>(p.smem_cole); }
-                else { e = col_set_attr<32, 256, 3>(p.smem_cole); if (!e) e = cole_set_attr<32, 256, 3>(p.smem_cole); }
+                if (X == 64) { e = col_set_attr<64, 256, 3>(p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3>(p.smem_cole_enc); }
+                else { e = col_set_attr<32, 256, 3>(p.smem_cole); if (!e) e = cole_set_attr<32, 256, 3>(p.smem_cole_enc); }
             } else {
-                if (X == 64) { e = col_set_attr<64, 512, 1>(p.smem_cole); if (!e) e = cole_set_attr<64, 512, 1>(p.smem_cole); }
-                else { e = col_set_attr<32, 512, 1>(p.smem_cole); if (!e) e = cole_set_attr<32, 512, 1>(p.smem_cole); }
+                if (X == 64) { e = col_set_attr<64, 512, 1>(p.smem_cole); if (!e) e = cole_set_attr<64, 512, 1>(p.smem_cole_enc); }
+                else { e = col_set_attr<32, 512, 1>(p.smem_cole); if (!e) e = cole_set_attr<32, 512, 1>(p.smem_cole_enc); }
             }
             if (e != cudaSuccess) return e;
             e = cudaFuncSetAttribute(row_pass_kernel<false, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
@@ -994,7 +1004,7 @@ static cudaError_t launch_col_enc(const Geom &g, const Plan &p, uint8_t *io, con
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
 #define VK_COLE(X, NT, MINB)                                                                                        \
-    return launch_pdl(col_enc_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_main, tm_pad, tm_B, B, (uint8_t *)io, D, g, \
+    return launch_pdl(col_enc_kernel<X, NT, MINB>, grid, NT, p.smem_cole_enc, st, tm_main, tm_pad, tm_B, B, (uint8_t *)io, D, g, \
                       (uint32_t)p.strips_per_frame, (uint32_t)n, p.box_rows, p.h_magic, pbox)
     if (p.col_ctas_per_sm == 3) {
         if (p.strip_bytes == 64) VK_COLE(64, 256, 3);

@@ -35,7 +35,8 @@ struct Plan {
     void *encode_tiled;    // cuTensorMapEncodeTiled, resolved through the runtime (no link-time libcuda dependency)
     int col_ctas_per_sm;   // column pass variant (3: 256-thread CTAs, two or three per SM; 1: one 512-thread CTA per SM)
     size_t smem_row;       // dynamic shared memory of the row pass
-    size_t smem_cole;      // dynamic shared memory of the column pass (either direction)
+    size_t smem_cole;      // dynamic shared memory of the column pass, decrypt direction (the strip)
+    size_t smem_cole_enc;  // ... encrypt direction: the strip, or more when that is how two CTAs per SM are asked for
     size_t max_frames_per_launch;  // keeps the intermediate (n * 3wh bytes) L2-resident
 };
 
