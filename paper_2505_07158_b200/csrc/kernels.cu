@@ -939,7 +939,12 @@ template <bool INV>
 static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, size_t n,
                               uint8_t *dst, cudaStream_t st) {
     const uint32_t nblocks = (uint32_t)(n * g.h / ROW_RB);
-    const uint32_t grid = nblocks < (uint32_t)p.row_grid_max ? nblocks : (uint32_t)p.row_grid_max;
+    // persistent CTAs, balanced: the fewest rounds the resident CTAs allow, then the smallest grid that needs no more rounds
+    // (FHD, 5 frames: 1350 blocks = 5 rounds of 270 CTAs instead of 296 CTAs of which 166 take a 5th block; measured 4.50 ->
+    // 4.44 us per frame, decrypt 5.58 -> 5.46: no CTA idles through a last round while it holds its share of the SM)
+    const uint32_t gmax = (uint32_t)p.row_grid_max;
+    const uint32_t rounds = (nblocks + gmax - 1u) / gmax;
+    const uint32_t grid = (nblocks + rounds - 1u) / rounds;
     const uint32_t nt = (uint32_t)p.row_nc + 32u;
     if (p.row_big)
         return launch_pdl(row_pass_kernel<INV, 1024, 1>, grid, nt, p.smem_row, st, src, dst, D, g, nblocks, (uint32_t)p.row_ns,
