@@ -60,6 +60,7 @@ extern "C" {
 #define VCRYPT_FLAG_HOST_SCALAR 4u    /* host derivation without SHA-NI / AVX lanes (test hook)   */
 #define VCRYPT_FLAG_DEVICE_DERIVE 8u  /* worker systems -> D, B on the GPU (same bytes): the host only
                                          hashes and runs the serial LHCS_m chain; D and B never cross PCIe */
+#define VCRYPT_FLAG_PERSISTENT 32u    /* one persistent kernel per call (cipher.cu: row team + strip team per SM) instead of the row-pass / column-pass kernel pairs */
 #define VCRYPT_FLAG_DEVICE_HASH 16u   /* sub-frame SHA-256 of vcrypt_encrypt_frames on the GPU, on the frames it
                                          uploads anyway, shared with the host threads band by band (device_hash_bands;
                                          same H); shapes with 3W % 16 != 0 are hashed on the host only */
@@ -86,6 +87,11 @@ typedef struct vcrypt_params {
                                so that one pair's column pass overlaps the next pair's row pass.  0 -> from the frame
                                size (about 31 MB of frames per pair when encrypting, 37 MB when decrypting).  Does not affect results                     */
     uint32_t pipe_streams;  /* 0 -> 2; 1 -> off (every launch on the caller's stream); at most 4                    */
+    /* tuning of the persistent cipher kernel (0 -> chosen from the frame size); none of them affects results */
+    uint32_t tune_row_stages;      /* input stages of the row team's shared-memory ring                            */
+    uint32_t tune_row_item_blocks; /* blocks of 4 rows per row ticket                                              */
+    uint32_t tune_window;          /* frames the leading pass may run ahead of the following one (0 -> 4)          */
+    uint32_t tune_ring;            /* chunks of the strip team's keystream ring in shared memory (1, 2; 3: none)   */
 } vcrypt_params;
 
 /* Algorithm 1 set-up (PAPER.md:85 steps 1-2): validates the parameters, whitens the key (reading Q5 of

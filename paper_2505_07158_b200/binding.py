@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 OK, E_ARG, E_KEY, E_SHAPE, E_CUDA, E_NOMEM, E_STATE = 0, -1, -2, -3, -4, -5, -6
-FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR, FLAG_DEVICE_DERIVE, FLAG_DEVICE_HASH = 1, 2, 4, 8, 16
+FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR, FLAG_DEVICE_DERIVE, FLAG_DEVICE_HASH, FLAG_PERSISTENT = 1, 2, 4, 8, 16, 32
 
 
 class Params(C.Structure):
@@ -22,7 +22,9 @@ class Params(C.Structure):
                 ("gamma", C.c_double), ("n_workers", C.c_uint32), ("width", C.c_uint32), ("height", C.c_uint32),
                 ("batch", C.c_uint32), ("n_streams", C.c_uint32), ("host_threads", C.c_uint32),
                 ("flags", C.c_uint32), ("device", C.c_int32), ("device_hash_bands", C.c_uint32),
-                ("pipe_frames", C.c_uint32), ("pipe_streams", C.c_uint32)]
+                ("pipe_frames", C.c_uint32), ("pipe_streams", C.c_uint32),
+                ("tune_row_stages", C.c_uint32), ("tune_row_item_blocks", C.c_uint32), ("tune_window", C.c_uint32),
+                ("tune_ring", C.c_uint32)]
 
 
 class FrameStats(C.Structure):
@@ -108,14 +110,14 @@ class Vcrypt:
 
     def __init__(self, key, gamma: float, n_workers: int, width: int, height: int, batch: int = 0,
                  n_streams: int = 0, host_threads: int = 0, flags: int = 0, device: int = -1, device_hash_bands: int = 0,
-                 pipe_frames: int = 0, pipe_streams: int = 0):
+                 pipe_frames: int = 0, pipe_streams: int = 0, tune=(0, 0, 0, 0)):
         self.L = lib()
         self.w, self.h, self.n = int(width), int(height), int(n_workers)
         self.frame_bytes = 3 * self.w * self.h
         self.nD = 3 * (self.w + self.h)
         x0, y0, z0, w0 = (float(v) for v in key)
         self.params = Params(x0, y0, z0, w0, float(gamma), n_workers, width, height, batch, n_streams,
-                             host_threads, flags, device, device_hash_bands, pipe_frames, pipe_streams)
+                             host_threads, flags, device, device_hash_bands, pipe_frames, pipe_streams, *[int(t) for t in (tuple(tune) + (0,) * 4)[:4]])
         self._p = _vp()
         rc = self.L.vcrypt_init(C.byref(self._p), C.byref(self.params))
         if rc != OK:

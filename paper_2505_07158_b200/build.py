@@ -22,7 +22,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 CXX_FLAGS = ["-O3", "-std=c++17", "-fPIC", "-ffp-contract=off", "-fno-fast-math", "-Wall", "-Wextra",
              "-fvisibility=hidden", f"-I{CUDA_HOME}/include"]
 # (source, extra flags); derive.cu holds the chaotic-map arithmetic: no FMA contraction
-CU_SOURCES = [("kernels.cu", []), ("membench.cu", []), ("derive.cu", ["-fmad=false"]), ("sha256.cu", []), ("stats.cu", [])]
+CU_SOURCES = [("kernels.cu", []), ("cipher.cu", []), ("membench.cu", []), ("derive.cu", ["-fmad=false"]), ("sha256.cu", []), ("stats.cu", [])]
 # (source, extra flags)
 CXX_SOURCES = [
     ("vcrypt.cpp", []),
@@ -32,7 +32,7 @@ CXX_SOURCES = [
     ("host_lhcs_avx2.cpp", ["-mavx2"]),
     ("host_lhcs_avx512.cpp", ["-mavx512f", "-mavx512dq", "-mprefer-vector-width=512"]),
 ]
-HEADERS = ["host.hpp", "kernels.cuh", "thread_pool.hpp", "host_lhcs_lanes.inc", os.path.join("..", "..", "include", "vcrypt.h")]
+HEADERS = ["host.hpp", "kernels.cuh", "ptx.cuh", "thread_pool.hpp", "host_lhcs_lanes.inc", os.path.join("..", "..", "include", "vcrypt.h")]
 
 
 def _nvcc() -> str:

@@ -50,6 +50,45 @@ cudaError_t encrypt_tiled(const Geom &g, const Plan &p, const uint8_t *src, cons
 cudaError_t decrypt_tiled(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, const uint8_t *B,
                           size_t n, uint8_t *dst, cudaStream_t st, int *launches);
 
+// ---------------------------------------------------------------------------------------------
+// The persistent cipher kernel (cipher.cu): row items and strip items of one call taken by ticket from one launch.
+// ---------------------------------------------------------------------------------------------
+struct UniTune {               // 0 = chosen from the shape; none of them affects results
+    uint32_t row_stages;       // input stages of the row ring
+    uint32_t row_item_blocks;  // blocks of 4 rows per row ticket
+    uint32_t window;           // frames the leading pass may be ahead of the following one
+    uint32_t ring;             // chunks of the strip team's keystream ring (1, 2; 3: none)
+};
+
+struct UniPlan {
+    bool ok;               // shape takes the tiled path (w % 16 == 0, w >= 64, h % 4 == 0, h >= 16, a strip and a row ring fit in shared memory)
+    int X;                 // byte columns per strip (64, or 32 for very tall frames)
+    int ns, nob;           // row team: input stages, output buffers
+    int bpi;               // row team: blocks per ticket
+    int grid_max;          // resident CTAs (one per SM)
+    int nring;             // strip team: chunks of the keystream ring
+    uint32_t strip_off;    // byte offset of the strip in the dynamic shared memory
+    uint32_t bring_off;    // ... of the keystream ring
+    size_t smem;           // dynamic shared memory per CTA
+    uint32_t nblk;         // blocks of 4 rows per frame
+    uint32_t row_items;    // row tickets per frame
+    uint32_t strips;       // per frame
+    uint32_t window;
+    uint32_t box_rows;     // rows per TMA tensor tile of a strip (largest divisor of h that is <= 256)
+    uint32_t h_magic;      // ceil(2^32 / h): d mod h without a division for d < 2^16
+    void *encode_tiled;    // cuTensorMapEncodeTiled, resolved through the runtime (no link-time libcuda dependency)
+};
+
+cudaError_t make_uni_plan(const Geom &g, int device, const UniTune &tune, UniPlan *out);
+
+// Words of launch state cipher_launch needs for n frames (zero before the first use; the kernel leaves it zero).
+inline size_t cipher_sched_words(size_t n) { return 4 + 2 * n; }
+
+// Encrypt (row items lead, strip items follow) or decrypt (strip items lead) n frames with ONE launch on `st`.
+// dst may equal src.  `sched`: device, cipher_sched_words(n) zeroed words, not shared with a launch that may run concurrently.
+cudaError_t cipher_launch(const Geom &g, const UniPlan &p, bool decrypt, const uint8_t *src, const uint16_t *D, const uint8_t *B,
+                          size_t n, uint8_t *dst, uint32_t *sched, cudaStream_t st);
+
 // Any-shape path: one thread per output byte, closed-form gather straight from global memory.
 // dst must not alias src.
 cudaError_t encrypt_generic(const Geom &g, const uint8_t *src, const uint16_t *D, const uint8_t *B, size_t n,

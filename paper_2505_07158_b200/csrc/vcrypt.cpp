@@ -77,6 +77,13 @@ struct vcrypt_ctx {
     int pipe_streams = 2;
     cudaStream_t pipe_st[kPipeMax - 1] = {nullptr, nullptr, nullptr};
     cudaEvent_t pipe_fork = nullptr, pipe_join[kPipeMax - 1] = {nullptr, nullptr, nullptr};
+    // persistent cipher kernel (cipher.cu): plan + launch state, one buffer per stream that calls on this context arrive on
+    vk::UniPlan uni{};
+    static constexpr int kSchedSlots = 32;
+    static constexpr size_t kSchedFrames = 4096;  // frames per launch at most (longer calls are cut)
+    uint32_t *d_sched = nullptr;                  // kSchedSlots x cipher_sched_words(kSchedFrames), zero between launches
+    cudaStream_t sched_owner[kSchedSlots] = {};
+    int sched_n = 0;
     // generic-path scratch for in-place calls
     uint8_t *d_scratch = nullptr;
     size_t scratch_bytes = 0;
@@ -199,12 +206,43 @@ int retire_slot(vcrypt_ctx *c, Slot &s) {
     return VCRYPT_OK;
 }
 
+// Launch state of the persistent cipher kernel for work enqueued on `st`: launches on one stream follow each other (the
+// kernel waits for its predecessor before it touches the state and leaves it zeroed), so one buffer per stream is enough.
+int sched_for_stream(vcrypt_ctx *c, cudaStream_t st, uint32_t **out) {
+    const size_t words = vk::cipher_sched_words(vcrypt_ctx::kSchedFrames);
+    if (!c->d_sched) {
+        VC_CUDA(c, cudaMalloc(&c->d_sched, vcrypt_ctx::kSchedSlots * words * sizeof(uint32_t)));
+        VC_CUDA(c, cudaMemset(c->d_sched, 0, vcrypt_ctx::kSchedSlots * words * sizeof(uint32_t)));
+    }
+    for (int i = 0; i < c->sched_n; ++i)
+        if (c->sched_owner[i] == st) { *out = c->d_sched + (size_t)i * words; return VCRYPT_OK; }
+    if (c->sched_n == vcrypt_ctx::kSchedSlots) {  // more streams than buffers: wait for everything, start over
+        VC_CUDA(c, cudaDeviceSynchronize());
+        c->sched_n = 0;
+    }
+    c->sched_owner[c->sched_n] = st;
+    *out = c->d_sched + (size_t)c->sched_n * words;
+    c->sched_n += 1;
+    return VCRYPT_OK;
+}
+
 int launch_cipher(vcrypt_ctx *c, bool decrypt, const uint8_t *src, const uint16_t *D, const uint8_t *B, size_t n,
                   uint8_t *dst, cudaStream_t st) {
     int launches = 0;
     cudaError_t e;
     const bool aligned = ((((uintptr_t)src) | ((uintptr_t)dst) | ((uintptr_t)B)) & 15u) == 0;
-    if (c->plan.tiled && aligned && !(c->p.flags & VCRYPT_FLAG_FORCE_GENERIC)) {
+    if (c->uni.ok && aligned && (c->p.flags & VCRYPT_FLAG_PERSISTENT) && !(c->p.flags & VCRYPT_FLAG_FORCE_GENERIC)) {
+        // one persistent kernel per call (per kSchedFrames frames): row items and strip items taken by ticket (cipher.cu)
+        uint32_t *sched = nullptr;
+        const int rs = sched_for_stream(c, st, &sched);
+        if (rs != VCRYPT_OK) return rs;
+        e = cudaSuccess;
+        for (size_t f0 = 0; f0 < n && e == cudaSuccess; f0 += vcrypt_ctx::kSchedFrames) {
+            const size_t m = n - f0 < vcrypt_ctx::kSchedFrames ? n - f0 : vcrypt_ctx::kSchedFrames, off = f0 * c->g.frame_bytes;
+            e = vk::cipher_launch(c->g, c->uni, decrypt, src + off, D + f0 * c->g.nD, B + off, m, dst + off, sched, st);
+            if (e == cudaSuccess) ++launches;
+        }
+    } else if (c->plan.tiled && aligned && !(c->p.flags & VCRYPT_FLAG_FORCE_GENERIC)) {
         const size_t pf = c->pipe_frames[decrypt ? 1 : 0];
         if (c->pipe_streams >= 2 && n >= 4 * pf) {  // fewer pairs never reach a steady state: the fork / join costs more than it hides
             // Resident clip.  The two passes of a launch pair stress different parts of the memory system (the row pass
@@ -322,6 +360,10 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
             if (dev < 0) e = cudaGetDevice(&dev);
             if (e == cudaSuccess) e = cudaSetDevice(dev);
             if (e == cudaSuccess) e = vk::make_plan(c->g, dev, &c->plan);
+            if (e == cudaSuccess) {
+                vk::UniTune tune{p->tune_row_stages, p->tune_row_item_blocks, p->tune_window, p->tune_ring};
+                e = vk::make_uni_plan(c->g, dev, tune, &c->uni);
+            }
             if (e != cudaSuccess) {
                 cudaGetLastError();
                 rc = VCRYPT_E_CUDA;
@@ -354,6 +396,10 @@ extern "C" void vcrypt_destroy(vcrypt_ctx *c) {
             if (c->pipe_join[i]) cudaEventDestroy(c->pipe_join[i]);
         }
         if (c->pipe_fork) cudaEventDestroy(c->pipe_fork);
+        if (c->d_sched) {
+            cudaDeviceSynchronize();
+            cudaFree(c->d_sched);
+        }
         if (c->d_scratch) {
             cudaDeviceSynchronize();
             cudaFree(c->d_scratch);
