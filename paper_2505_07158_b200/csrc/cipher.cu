@@ -53,7 +53,14 @@ constexpr int ROW_MAXNS = 8;     // input stages at most
 constexpr int ROW_MAXOB = 2;     // output buffers at most
 constexpr int CE_PAD = 8;        // repeated strip rows
 constexpr int CE_G = 8;          // output rows per group
-constexpr int NRW = 8;           // row team: compute warps
+#ifndef VK_NRW
+#define VK_NRW 8
+#endif
+#ifndef VK_NSW
+#define VK_NSW 12
+#endif
+constexpr int NRW = VK_NRW;      // row team: compute warps
+constexpr int NSW = VK_NSW;      // strip team: compute warps
 constexpr uint32_t DESC_TERM = 0xFFFFFFFFu, DESC_LAST = 0x80000000u;
 
 // Per-item timeline for development builds (-DVK_TRACE; not part of the product)
@@ -748,8 +755,8 @@ __device__ __forceinline__ void strip_compute(const Smem &m, const UniArgs &a, c
 // The kernel: one persistent CTA per SM.  Warps 0 .. 7 row compute, 8 row load, 9 row store, 10 .. 10 + NSW - 1 strip
 // compute, 10 + NSW strip service.
 // ---------------------------------------------------------------------------------------------
-template <bool INV, int X, int NSW>
-__global__ void __launch_bounds__((NRW + NSW + 3) * 32, 1)
+template <bool INV, int X, int NSW_>
+__global__ void __launch_bounds__((NRW + NSW_ + 3) * 32, 1)
     cipher_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_pad,
                   const __grid_constant__ CUtensorMap tm_B, const UniArgs a) {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -761,7 +768,7 @@ __global__ void __launch_bounds__((NRW + NSW + 3) * 32, 1)
         mbar_init(m.sitem, 1);
         mbar_init(m.sbar, 1);
         mbar_init(m.sfree, 1);
-        for (uint32_t c = 0; c < 2; ++c) { mbar_init(m.bfull + c, 1); mbar_init(m.bfree + c, NSW * 32); }
+        for (uint32_t c = 0; c < 2; ++c) { mbar_init(m.bfull + c, 1); mbar_init(m.bfree + c, NSW_ * 32); }
         mbar_init_fence();
     }
     if (tid == 32) { tmap_prefetch(&tm_a); tmap_prefetch(&tm_pad); tmap_prefetch(&tm_B); }
@@ -772,8 +779,8 @@ __global__ void __launch_bounds__((NRW + NSW + 3) * 32, 1)
     if (warp < NRW) row_compute<INV>(m, a, tid);
     else if (warp == NRW) row_load_warp<INV>(m, a, lane);
     else if (warp == NRW + 1) row_store_warp(m, a, lane);
-    else if (warp < NRW + 2 + NSW) strip_compute<INV, X, NSW * 32>(m, a, &tm_B, tid - (NRW + 2) * 32);
-    else strip_service_warp<INV, X, NSW * 32>(m, a, &tm_a, &tm_pad, &tm_B, lane);
+    else if (warp < NRW + 2 + NSW_) strip_compute<INV, X, NSW_ * 32>(m, a, &tm_B, tid - (NRW + 2) * 32);
+    else strip_service_warp<INV, X, NSW_ * 32>(m, a, &tm_a, &tm_pad, &tm_B, lane);
 
     // the last CTA to leave restores the launch state for the next launch that uses this buffer
     __syncthreads();
@@ -805,9 +812,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-template <bool INV, int X, int NSW>
+template <bool INV, int X, int NSW_>
 static cudaError_t uni_attr(size_t smem) {
-    return cudaFuncSetAttribute(cipher_kernel<INV, X, NSW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return cudaFuncSetAttribute(cipher_kernel<INV, X, NSW_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
 }
 
 cudaError_t make_uni_plan(const Geom &g, int device, const UniTune &tune, UniPlan *out) {
@@ -827,7 +834,7 @@ cudaError_t make_uni_plan(const Geom &g, int device, const UniTune &tune, UniPla
         if (X) {
             // what is left beside the strip goes to the keystream ring (two chunks = two rounds of the strip team) and to the row
             // ring: at least two stages and one output buffer before the keystream ring gets its second chunk
-            const size_t chunk = (size_t)12 * (32 / (X / 8)) * CE_G * X;  // GSTEP * 8 rows x X bytes
+            const size_t chunk = (size_t)NSW * (32 / (X / 8)) * CE_G * X;  // GSTEP * 8 rows x X bytes
             const size_t room = (size_t)smem_optin - UNI_HDR - uni_strip_bytes(g, X);
             int ns = 1, nob = 1, nring = 0;
             const int want_ring = tune.ring == 3 ? 0 : (tune.ring ? (int)tune.ring : 2);
@@ -865,8 +872,8 @@ cudaError_t make_uni_plan(const Geom &g, int device, const UniTune &tune, UniPla
             if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
                 qres == cudaDriverEntryPointSuccess && fn) {
                 p.encode_tiled = fn;
-                if (X == 64) { e = uni_attr<false, 64, 12>(p.smem); if (!e) e = uni_attr<true, 64, 12>(p.smem); }
-                else { e = uni_attr<false, 32, 12>(p.smem); if (!e) e = uni_attr<true, 32, 12>(p.smem); }
+                if (X == 64) { e = uni_attr<false, 64, NSW>(p.smem); if (!e) e = uni_attr<true, 64, NSW>(p.smem); }
+                else { e = uni_attr<false, 32, NSW>(p.smem); if (!e) e = uni_attr<true, 32, NSW>(p.smem); }
                 if (e != cudaSuccess) return e;
                 p.ok = true;
             }
@@ -921,12 +928,12 @@ cudaError_t cipher_launch(const Geom &g, const UniPlan &p, bool decrypt, const u
     a.box_rows = p.box_rows; a.h_magic = p.h_magic; a.pf_rows = pbox;
     const uint64_t units = (uint64_t)n * (p.row_items < p.strips ? p.row_items : p.strips);
     const uint32_t grid = units < (uint64_t)p.grid_max ? (uint32_t)(units ? units : 1) : (uint32_t)p.grid_max;
-    const uint32_t block = (uint32_t)(NRW + 12 + 3) * 32u;
+    const uint32_t block = (uint32_t)(NRW + NSW + 3) * 32u;
     if (p.X == 64)
-        return decrypt ? launch_pdl(cipher_kernel<true, 64, 12>, grid, block, p.smem, st, tm_a, tm_pad, tm_B, a)
-                       : launch_pdl(cipher_kernel<false, 64, 12>, grid, block, p.smem, st, tm_a, tm_pad, tm_B, a);
-    return decrypt ? launch_pdl(cipher_kernel<true, 32, 12>, grid, block, p.smem, st, tm_a, tm_pad, tm_B, a)
-                   : launch_pdl(cipher_kernel<false, 32, 12>, grid, block, p.smem, st, tm_a, tm_pad, tm_B, a);
+        return decrypt ? launch_pdl(cipher_kernel<true, 64, NSW>, grid, block, p.smem, st, tm_a, tm_pad, tm_B, a)
+                       : launch_pdl(cipher_kernel<false, 64, NSW>, grid, block, p.smem, st, tm_a, tm_pad, tm_B, a);
+    return decrypt ? launch_pdl(cipher_kernel<true, 32, NSW>, grid, block, p.smem, st, tm_a, tm_pad, tm_B, a)
+                   : launch_pdl(cipher_kernel<false, 32, NSW>, grid, block, p.smem, st, tm_a, tm_pad, tm_B, a);
 }
 
 }  // namespace vk

@@ -39,6 +39,8 @@
 // (w % 16 != 0, w < 64, h % 4 != 0, h < 16, or a strip / row block too large for shared memory).
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "kernels.cuh"
 
 namespace vk {
@@ -341,6 +343,17 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
 // select per output word.
 // In place is safe: the whole strip is in shared memory before the first store.
 // ---------------------------------------------------------------------------------------------
+// keystream prefetch depths (rounds of loads in flight per thread): decrypt column pass with three CTAs per SM / one CTA per
+// SM, encrypt column pass with one CTA per SM (development builds may override)
+#ifndef VK_KD3
+#define VK_KD3 2
+#endif
+#ifndef VK_KD1
+#define VK_KD1 3
+#endif
+#ifndef VK_DE1
+#define VK_DE1 2
+#endif
 constexpr int CE_PAD = 8;   // repeated strip rows
 constexpr int CE_G = 8;     // output rows per group
 
@@ -367,7 +380,7 @@ __device__ __forceinline__ uint64_t mad_wide_ptr(const void *p, uint32_t off) {
     return r;
 }
 
-template <int X, int NT, int MINB>
+template <int X, int NT, int MINB, int DEPTH>
 __global__ void __launch_bounds__(NT, MINB)
     col_enc_kernel(const __grid_constant__ CUtensorMap tm_main, const __grid_constant__ CUtensorMap tm_pad,
                    const __grid_constant__ CUtensorMap tm_B, const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
@@ -391,7 +404,8 @@ __global__ void __launch_bounds__(NT, MINB)
     // ahead of the row group the CTA is working on (the threads' own loads then hit L2 instead of waiting on DRAM)
     uint32_t pf_row = 0;
     if (threadIdx.x == 0) {
-        for (; pf_row < h && pf_row < CE_AHEAD; pf_row += pf_rows) tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
+        for (; pf_row < h && pf_row < CE_AHEAD + (DEPTH - 1) * GSTEP * CE_G; pf_row += pf_rows)
+            tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
         mbar_init(bar, 1);
         pdl_wait();  // the strip is the row pass's output
         const uint64_t pol = policy_evict_first();
@@ -426,18 +440,26 @@ __global__ void __launch_bounds__(NT, MINB)
     const size_t gstep = (size_t)(GSTEP * CE_G) * rb;
 
 #define VK_ROWPTR(T, P, OFF) reinterpret_cast<T>(mad_wide_ptr(P, OFF))
-    // keystream of the first group: issued before the strip arrives
-    uint2 kb[CE_G];
+    // keystream of the first DEPTH groups: issued before the strip arrives (DEPTH = 2 where the registers are there: two
+    // rounds of loads in flight per thread, and two rounds of latency hidden)
+    uint2 kb[DEPTH][CE_G];
 #pragma unroll
-    for (int i = 0; i < CE_G; ++i) kb[i] = make_uint2(0u, 0u);
+    for (int d = 0; d < DEPTH; ++d)
+#pragma unroll
+        for (int i = 0; i < CE_G; ++i) kb[d][i] = make_uint2(0u, 0u);
     if (active) {
         const uint32_t offs[8] = {0u, rb, rb2, rb3, rb4, rb5, rb6, rb7};
-        if (g0 < nfull) {
 #pragma unroll
-            for (int i = 0; i < CE_G; ++i) kb[i] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[i]));
-        } else {
+        for (int d = 0; d < DEPTH; ++d) {
+            const uint32_t gd = g0 + (uint32_t)d * GSTEP;
+            const uint8_t *pd = pB + (size_t)d * gstep;
+            if (gd < nfull) {
 #pragma unroll
-            for (int i = 0; i < CE_G / 2; ++i) kb[i] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[i]));
+                for (int i = 0; i < CE_G; ++i) kb[d][i] = __ldcs(VK_ROWPTR(const uint2 *, pd, offs[i]));
+            } else if (gd * CE_G < h) {
+#pragma unroll
+                for (int i = 0; i < CE_G / 2; ++i) kb[d][i] = __ldcs(VK_ROWPTR(const uint2 *, pd, offs[i]));
+            }
         }
     }
     __syncthreads();  // mbarrier initialised, ups[] complete
@@ -477,66 +499,81 @@ __global__ void __launch_bounds__(NT, MINB)
     mbar_wait(bar, 0);  // strip (and its wrap rows) has landed: the previous kernel has completed (thread 0 waited for it)
     if (!active) return;
 
-    for (uint32_t gi = g0;; gi += GSTEP) {
-        uint32_t O[CE_G][2];
+    // one round = one group of 8 output rows of this lane's columns; PD = which keystream register set it uses (compile time)
+    uint32_t gi = g0;
+    auto round = [&](auto PD) -> bool {
+        constexpr int pd = decltype(PD)::value;
+        {
+            uint32_t O[CE_G][2];
 #pragma unroll
-        for (int al_ = 0; al_ < 2; ++al_) {
-            uint32_t A[4][2];
+            for (int al_ = 0; al_ < 2; ++al_) {
+                uint32_t A[4][2];
 #pragma unroll
-            for (int ab = 0; ab < 4; ++ab) {
-                const int a = al_ * 4 + ab;
-                const uint32_t Ka = (uint32_t)ab * X + 4u * (uint32_t)al_;
-                const uint8_t *p = S + ((q[a] & m3) ^ Ka);
-                const uint32_t r0 = *reinterpret_cast<const uint32_t *>(p);
-                const uint32_t r1 = *reinterpret_cast<const uint32_t *>(p + 4 * X);
-                const uint32_t r2 = *reinterpret_cast<const uint32_t *>(p + 8 * X);
-                const uint32_t shamt = q[a] << 3;  // funnel shift uses the low 5 bits: 8 * alignment
-                A[ab][0] = __funnelshift_r(r0, r1, shamt);
-                A[ab][1] = __funnelshift_r(r1, r2, shamt);
-                q[a] += ADVX;
-                if (q[a] >= hX) q[a] -= hX;
+                for (int ab = 0; ab < 4; ++ab) {
+                    const int a = al_ * 4 + ab;
+                    const uint32_t Ka = (uint32_t)ab * X + 4u * (uint32_t)al_;
+                    const uint8_t *p = S + ((q[a] & m3) ^ Ka);
+                    const uint32_t r0 = *reinterpret_cast<const uint32_t *>(p);
+                    const uint32_t r1 = *reinterpret_cast<const uint32_t *>(p + 4 * X);
+                    const uint32_t r2 = *reinterpret_cast<const uint32_t *>(p + 8 * X);
+                    const uint32_t shamt = q[a] << 3;  // funnel shift uses the low 5 bits: 8 * alignment
+                    A[ab][0] = __funnelshift_r(r0, r1, shamt);
+                    A[ab][1] = __funnelshift_r(r1, r2, shamt);
+                    q[a] += ADVX;
+                    if (q[a] >= hX) q[a] -= hX;
+                }
+#pragma unroll
+                for (int hg = 0; hg < 2; ++hg) {
+                    const uint32_t t01a = __byte_perm(A[0][hg], A[1][hg], selA), t01b = __byte_perm(A[0][hg], A[1][hg], selB);
+                    const uint32_t t23a = __byte_perm(A[2][hg], A[3][hg], selA), t23b = __byte_perm(A[2][hg], A[3][hg], selB);
+                    O[4 * hg + 0][al_] = __byte_perm(t01a, t23a, selLo);
+                    O[4 * hg + 1][al_] = __byte_perm(t01a, t23a, selHi);
+                    O[4 * hg + 2][al_] = __byte_perm(t01b, t23b, selLo);
+                    O[4 * hg + 3][al_] = __byte_perm(t01b, t23b, selHi);
+                }
             }
+            // undo the word column permutation, xor the keystream, store
+            const uint32_t offs[8] = {0u, rb, rb2, rb3, rb4, rb5, rb6, rb7};
+            if (gi < nfull) {
 #pragma unroll
-            for (int hg = 0; hg < 2; ++hg) {
-                const uint32_t t01a = __byte_perm(A[0][hg], A[1][hg], selA), t01b = __byte_perm(A[0][hg], A[1][hg], selB);
-                const uint32_t t23a = __byte_perm(A[2][hg], A[3][hg], selA), t23b = __byte_perm(A[2][hg], A[3][hg], selB);
-                O[4 * hg + 0][al_] = __byte_perm(t01a, t23a, selLo);
-                O[4 * hg + 1][al_] = __byte_perm(t01a, t23a, selHi);
-                O[4 * hg + 2][al_] = __byte_perm(t01b, t23b, selLo);
-                O[4 * hg + 3][al_] = __byte_perm(t01b, t23b, selHi);
+                for (int i = 0; i < CE_G; ++i) {
+                    const uint32_t lo = sl ? O[i][1] : O[i][0], hi = sl ? O[i][0] : O[i][1];
+                    __stcs(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[pd][i].x, hi ^ kb[pd][i].y));
+                }
+            } else {  // the half group at the bottom of a frame with h % 8 == 4: always the last one
+#pragma unroll
+                for (int i = 0; i < CE_G / 2; ++i) {
+                    const uint32_t lo = sl ? O[i][1] : O[i][0], hi = sl ? O[i][0] : O[i][1];
+                    __stcs(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[pd][i].x, hi ^ kb[pd][i].y));
+                }
+                return false;
             }
+            const uint32_t gn = gi + GSTEP;
+            if (gn * CE_G >= h) return false;
+            // keystream of the group DEPTH rounds on, into the registers just used
+            const uint32_t gl = gi + (uint32_t)DEPTH * GSTEP;
+            if (threadIdx.x == 0)
+                for (; pf_row < h && pf_row < gl * CE_G + CE_AHEAD; pf_row += pf_rows)
+                    tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
+            {
+                const uint8_t *pl = pB + (size_t)DEPTH * gstep;
+                if (gl < nfull) {
+#pragma unroll
+                    for (int i = 0; i < CE_G; ++i) kb[pd][i] = __ldcs(VK_ROWPTR(const uint2 *, pl, offs[i]));
+                } else if (gl * CE_G < h) {
+#pragma unroll
+                    for (int i = 0; i < CE_G / 2; ++i) kb[pd][i] = __ldcs(VK_ROWPTR(const uint2 *, pl, offs[i]));
+                }
+            }
+            pB += gstep;
+            pO += gstep;
+            gi = gn;
         }
-        // undo the word column permutation, xor the keystream, store
-        const uint32_t offs[8] = {0u, rb, rb2, rb3, rb4, rb5, rb6, rb7};
-        if (gi < nfull) {
-#pragma unroll
-            for (int i = 0; i < CE_G; ++i) {
-                const uint32_t lo = sl ? O[i][1] : O[i][0], hi = sl ? O[i][0] : O[i][1];
-                __stcs(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[i].x, hi ^ kb[i].y));
-            }
-        } else {  // the half group at the bottom of a frame with h % 8 == 4: always the last one
-#pragma unroll
-            for (int i = 0; i < CE_G / 2; ++i) {
-                const uint32_t lo = sl ? O[i][1] : O[i][0], hi = sl ? O[i][0] : O[i][1];
-                __stcs(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[i].x, hi ^ kb[i].y));
-            }
-            break;
-        }
-        // keystream of the next group
-        const uint32_t gn = gi + GSTEP;
-        if (gn * CE_G >= h) break;
-        if (threadIdx.x == 0)
-            for (; pf_row < h && pf_row < gn * CE_G + CE_AHEAD; pf_row += pf_rows)
-                tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
-        pB += gstep;
-        pO += gstep;
-        if (gn < nfull) {
-#pragma unroll
-            for (int i = 0; i < CE_G; ++i) kb[i] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[i]));
-        } else {
-#pragma unroll
-            for (int i = 0; i < CE_G / 2; ++i) kb[i] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs[i]));
-        }
+        return true;
+    };
+    for (;;) {
+        if (!round(std::integral_constant<int, 0>{})) break;
+        if (DEPTH > 1 && !round(std::integral_constant<int, DEPTH - 1>{})) break;
     }
 #undef VK_ROWPTR
 }
@@ -553,7 +590,7 @@ __global__ void __launch_bounds__(NT, MINB)
 // a half warp sit in disjoint banks).
 // In place (dst == src) is safe: the whole strip is in shared memory (barrier) before the first store.
 // ---------------------------------------------------------------------------------------------
-template <int X, int NT, int MINB>
+template <int X, int NT, int MINB, int KD>
 __global__ void __launch_bounds__(NT, MINB)
     col_dec_kernel(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ CUtensorMap tm_B,
                    const uint8_t *__restrict__ Bk, uint8_t *dst, const uint16_t *__restrict__ D, Geom g,
@@ -575,7 +612,8 @@ __global__ void __launch_bounds__(NT, MINB)
     constexpr uint32_t CD_AHEAD = 2u * 4u * GSTEP;  // two iterations (measured: 1 -> 6.93, 2 -> 6.78, 4 -> 6.95 us per FHD frame)
     uint32_t pf_row = 0;
     if (threadIdx.x == 0) {
-        for (; pf_row < h && pf_row < CD_AHEAD; pf_row += pf_rows) tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
+        for (; pf_row < h && pf_row < CD_AHEAD + (KD - 1) * 4u * GSTEP; pf_row += pf_rows)
+            tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
         mbar_init(bar, 1);
         pdl_wait();  // the ciphertext may be the previous kernel's output
         const uint64_t pol = policy_evict_first();
@@ -611,32 +649,38 @@ __global__ void __launch_bounds__(NT, MINB)
     const uint32_t nblk = h >> 2;
     const uint32_t offs4[4] = {s1 ? rb : 0u, s1 ? 0u : rb, s1 ? rb3 : rb2, s1 ? rb2 : rb3};
     const uint8_t *pB = Bk + fcol + (size_t)(4u * g0) * rb;
-    uint2 kn[4];
+    // keystream of the first KD blocks of this sub-warp: issued before the strip arrives (KD blocks of loads in flight per thread)
+    const size_t bstep = (size_t)(4u * GSTEP) * rb;
+    uint2 kq[KD][4];
 #pragma unroll
-    for (int t = 0; t < 4; ++t) kn[t] = make_uint2(0u, 0u);
-    if (col_ok && g0 < nblk) {  // keystream of the first block: issued before the strip arrives
+    for (int d = 0; d < KD; ++d) {
 #pragma unroll
-        for (int t = 0; t < 4; ++t) kn[t] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs4[t]));
+        for (int t = 0; t < 4; ++t) kq[d][t] = make_uint2(0u, 0u);
+        if (col_ok && g0 + (uint32_t)d * GSTEP < nblk) {
+#pragma unroll
+            for (int t = 0; t < 4; ++t) kq[d][t] = __ldcs(VK_ROWPTR(const uint2 *, pB + (size_t)d * bstep, offs4[t]));
+        }
     }
     __syncthreads();    // mbarrier initialised, ups[] complete
     mbar_wait(bar, 0);  // the ciphertext strip has landed
     if (col_ok) {
         const uint32_t selA = s1 ? 0x1504u : 0x5140u, selB = s1 ? 0x3726u : 0x7362u;  // inputs arrive as rows (t ^ s1)
         const uint32_t selF = s1 ? 0x7632u : 0x5410u, selS = s1 ? 0x5410u : 0x7632u;  // first / second byte lane of a pair
-        const size_t bstep = (size_t)(4u * GSTEP) * rb;
         const int32_t d1 = s1 ? -(int32_t)X : (int32_t)X;
-        for (uint32_t R4 = g0; R4 < nblk; R4 += GSTEP) {
+        uint32_t R4 = g0;
+        auto block = [&](auto PD) {
+            constexpr int pd = decltype(PD)::value;
             uint2 k[4];
 #pragma unroll
-            for (int t = 0; t < 4; ++t) k[t] = kn[t];
-            pB += bstep;
+            for (int t = 0; t < 4; ++t) k[t] = kq[pd][t];
             if (threadIdx.x == 0)
-                for (; pf_row < h && pf_row < 4u * (R4 + GSTEP) + CD_AHEAD; pf_row += pf_rows)
+                for (; pf_row < h && pf_row < 4u * (R4 + (uint32_t)KD * GSTEP) + CD_AHEAD; pf_row += pf_rows)
                     tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
-            if (R4 + GSTEP < nblk) {
+            if (R4 + (uint32_t)KD * GSTEP < nblk) {  // the block KD rounds on, into the registers just read
 #pragma unroll
-                for (int t = 0; t < 4; ++t) kn[t] = __ldcs(VK_ROWPTR(const uint2 *, pB, offs4[t]));
+                for (int t = 0; t < 4; ++t) kq[pd][t] = __ldcs(VK_ROWPTR(const uint2 *, pB + (size_t)KD * bstep, offs4[t]));
             }
+            pB += bstep;
             uint8_t *ps = S + ((size_t)(4u * R4) * X + 8u * j) + (s1 ? X : 0u);
             uint2 v[4];
             v[0] = *reinterpret_cast<const uint2 *>(ps);
@@ -671,6 +715,12 @@ __global__ void __launch_bounds__(NT, MINB)
                 *reinterpret_cast<uint2 *>(pw + 2 * X) = make_uint2(lo[2], hi[2]);
                 *reinterpret_cast<uint2 *>(pw + 2 * X + d1) = make_uint2(lo[3], hi[3]);
             }
+            R4 += GSTEP;
+        };
+        while (R4 < nblk) {
+            block(std::integral_constant<int, 0>{});
+            if (KD > 1 && R4 < nblk) block(std::integral_constant<int, (KD > 1 ? 1 : 0)>{});
+            if (KD > 2 && R4 < nblk) block(std::integral_constant<int, (KD > 2 ? 2 : 0)>{});
         }
     }
     __syncthreads();  // strip and ups[] complete
@@ -811,13 +861,13 @@ static size_t row_smem_bytes(const Geom &g, int ns) {
 }
 static size_t cole_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + CE_PAD) * X + 16 + 2 * (size_t)X; }
 
-template <int X, int NT, int MINB>
+template <int X, int NT, int MINB, int KD>
 static cudaError_t col_set_attr(size_t smem) {
-    return cudaFuncSetAttribute(col_dec_kernel<X, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return cudaFuncSetAttribute(col_dec_kernel<X, NT, MINB, KD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
 }
-template <int X, int NT, int MINB>
+template <int X, int NT, int MINB, int DEPTH>
 static cudaError_t cole_set_attr(size_t smem) {
-    return cudaFuncSetAttribute(col_enc_kernel<X, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return cudaFuncSetAttribute(col_enc_kernel<X, NT, MINB, DEPTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -900,11 +950,11 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
             const size_t l2_budget = (size_t)100 << 20;
             p.max_frames_per_launch = l2_budget / g.frame_bytes ? l2_budget / g.frame_bytes : 1;
             if (ctas == 3) {
-                if (X == 64) { e = col_set_attr<64, 256, 3>(p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3>(p.smem_cole_enc); }
-                else { e = col_set_attr<32, 256, 3>(p.smem_cole); if (!e) e = cole_set_attr<32, 256, 3>(p.smem_cole_enc); }
+                if (X == 64) { e = col_set_attr<64, 256, 3, VK_KD3>(p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3, 1>(p.smem_cole_enc); if (!e) e = cole_set_attr<64, 256, 2, 2>(p.smem_cole_enc); }
+                else { e = col_set_attr<32, 256, 3, VK_KD3>(p.smem_cole); if (!e) e = cole_set_attr<32, 256, 3, 1>(p.smem_cole_enc); }
             } else {
-                if (X == 64) { e = col_set_attr<64, 512, 1>(p.smem_cole); if (!e) e = cole_set_attr<64, 512, 1>(p.smem_cole_enc); }
-                else { e = col_set_attr<32, 512, 1>(p.smem_cole); if (!e) e = cole_set_attr<32, 512, 1>(p.smem_cole_enc); }
+                if (X == 64) { e = col_set_attr<64, 512, 1, VK_KD1>(p.smem_cole); if (!e) e = cole_set_attr<64, 512, 1, VK_DE1>(p.smem_cole_enc); }
+                else { e = col_set_attr<32, 512, 1, VK_KD1>(p.smem_cole); if (!e) e = cole_set_attr<32, 512, 1, VK_DE1>(p.smem_cole_enc); }
             }
             if (e != cudaSuccess) return e;
             e = cudaFuncSetAttribute(row_pass_kernel<false, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
@@ -971,15 +1021,15 @@ static cudaError_t launch_col_dec(const Geom &g, const Plan &p, const uint8_t *s
     const uint32_t pbox = 64;  // look-ahead tile height (rows)
     if (!make_tmap(p, g, src, n, p.box_rows, &tm_src) || !make_tmap(p, g, B, n, pbox, &tm_B)) return cudaErrorInvalidValue;
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
-#define VK_COLD(X, NT, MINB)                                                                                         \
-    return launch_pdl(col_dec_kernel<X, NT, MINB>, grid, NT, p.smem_cole, st, tm_src, tm_B, B, dst, D, g,           \
+#define VK_COLD(X, NT, MINB, KD)                                                                                     \
+    return launch_pdl(col_dec_kernel<X, NT, MINB, KD>, grid, NT, p.smem_cole, st, tm_src, tm_B, B, dst, D, g,           \
                       (uint32_t)p.strips_per_frame, p.h_magic, p.box_rows, pbox)
     if (p.col_ctas_per_sm == 3) {
-        if (p.strip_bytes == 64) VK_COLD(64, 256, 3);
-        else VK_COLD(32, 256, 3);
+        if (p.strip_bytes == 64) VK_COLD(64, 256, 3, VK_KD3);
+        else VK_COLD(32, 256, 3, VK_KD3);
     } else {
-        if (p.strip_bytes == 64) VK_COLD(64, 512, 1);
-        else VK_COLD(32, 512, 1);
+        if (p.strip_bytes == 64) VK_COLD(64, 512, 1, VK_KD1);
+        else VK_COLD(32, 512, 1, VK_KD1);
     }
 #undef VK_COLD
     return cudaGetLastError();
@@ -1008,15 +1058,17 @@ static cudaError_t launch_col_enc(const Geom &g, const Plan &p, uint8_t *io, con
                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     const uint32_t grid = (uint32_t)(n * p.strips_per_frame);
-#define VK_COLE(X, NT, MINB)                                                                                        \
-    return launch_pdl(col_enc_kernel<X, NT, MINB>, grid, NT, p.smem_cole_enc, st, tm_main, tm_pad, tm_B, B, (uint8_t *)io, D, g, \
+#define VK_COLE(X, NT, MINB, DEPTH)                                                                                 \
+    return launch_pdl(col_enc_kernel<X, NT, MINB, DEPTH>, grid, NT, p.smem_cole_enc, st, tm_main, tm_pad, tm_B, B, (uint8_t *)io, D, g, \
                       (uint32_t)p.strips_per_frame, (uint32_t)n, p.box_rows, p.h_magic, pbox)
     if (p.col_ctas_per_sm == 3) {
-        if (p.strip_bytes == 64) VK_COLE(64, 256, 3);
-        else VK_COLE(32, 256, 3);
+        // two CTAs per SM (the larger shared-memory request): registers for two rounds of keystream in flight per thread
+        if (p.strip_bytes == 64 && p.smem_cole_enc != p.smem_cole) VK_COLE(64, 256, 2, 2);
+        else if (p.strip_bytes == 64) VK_COLE(64, 256, 3, 1);
+        else VK_COLE(32, 256, 3, 1);
     } else {
-        if (p.strip_bytes == 64) VK_COLE(64, 512, 1);
-        else VK_COLE(32, 512, 1);
+        if (p.strip_bytes == 64) VK_COLE(64, 512, 1, VK_DE1);
+        else VK_COLE(32, 512, 1, VK_DE1);
     }
 #undef VK_COLE
     return cudaGetLastError();
