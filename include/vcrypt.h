@@ -49,7 +49,7 @@ extern "C" {
 #define VCRYPT_OK 0
 #define VCRYPT_E_ARG (-1)    /* null pointer, zero size, misaligned device pointer   */
 #define VCRYPT_E_KEY (-2)    /* non-finite key word or gamma outside [-1.52, -0.06]  */
-#define VCRYPT_E_SHAPE (-3)  /* width/height/n_workers zero or too large             */
+#define VCRYPT_E_SHAPE (-3)  /* width/height/n_workers zero or too large (3*W*H < 2^31) */
 #define VCRYPT_E_CUDA (-4)   /* CUDA error, or GPU call on a host-only context       */
 #define VCRYPT_E_NOMEM (-5)  /* host or device allocation failed                     */
 #define VCRYPT_E_STATE (-6)  /* chaotic state left the finite range                  */
@@ -137,7 +137,7 @@ int vcrypt_derive(vcrypt_ctx *ctx, const uint8_t *hash, uint16_t *D_out, uint8_t
 /* The chain state = last LHCS_m record (x_2n, y_2n, z_2n, w_2n) and the number of frames
  * derived so far: 4 doubles + 1 counter are all a caller needs to checkpoint / resume a stream. */
 int vcrypt_get_state(const vcrypt_ctx *ctx, double state_out[4], uint64_t *frames_done);
-int vcrypt_set_state(vcrypt_ctx *ctx, const double state[4], uint64_t frames_done);
+int vcrypt_set_state(vcrypt_ctx *ctx, const double state[4], uint64_t frames_done); /* VCRYPT_E_STATE unless finite and |v| < 2^53 */
 
 /* Host threads actually started (the `cores` of a CPU-side figure). */
 int vcrypt_host_threads(const vcrypt_ctx *ctx);
@@ -211,26 +211,6 @@ int vcrypt_npcr_uaci_device(vcrypt_ctx *ctx, const void *d_a, const void *d_b, s
  * out: host, n x 3 doubles.  VCRYPT_E_ARG if a block leaves the frame. */
 int vcrypt_local_entropy_device(vcrypt_ctx *ctx, const void *d_frames, size_t n, const uint32_t *blocks_xy, uint32_t k,
                                 uint32_t side, double *out, void *cuda_stream);
-
-/* Memory-system probe (bench hook): moves the bytes of one vcrypt_encrypt_device call on `frames` frames of this
- * context's shape with no cipher arithmetic, `reps` times on the context's device, and returns the mean time of
- * one repetition in microseconds (CUDA events).  which = 0: sequential copy (read 3wh + write 3wh per frame);
- * 1: the traffic of any two-pass design, sequential (pass 1 reads F and writes an L2-resident intermediate,
- * pass 2 reads it back, reads B, writes the result: 5 trips through L2 per byte; cf. DESIGN.md "What bounds the
- * path"); 2: read B + write result in 64-byte-wide column strips (the DRAM side of the column pass).
- * Allocates and frees about 3.6 GB of device memory.  VCRYPT_E_ARG for a bad `which`, frames = 0 or reps < 1. */
-int vcrypt_memory_probe(vcrypt_ctx *ctx, int which, size_t frames, int reps, double *us_per_rep);
-
-/* Distributed-shared-memory exchange probe (design hook): as many thread-block clusters of
- * `cluster_size` CTAs (1 .. 16; sizes above 8 are non-portable) as are resident at once, every CTA owning
- * `bytes_per_cta` bytes of shared memory (a multiple of 16 x cluster_size; twice that + 64 must fit the per-CTA
- * limit); per round every CTA sends bytes_per_cta / cluster_size bytes to each CTA of its cluster -- one all-to-all
- * of cluster_size x bytes_per_cta bytes per cluster -- with 16-byte st.shared::cluster stores (mode 0) or
- * cp.async.bulk shared -> peer shared with mbarrier completion (mode 1).  Returns the mean time of one round in
- * microseconds (CUDA events, `rounds` rounds in one launch, cluster barrier per round) and the number of resident
- * clusters.  VCRYPT_E_ARG for sizes that do not fit. */
-int vcrypt_dsmem_probe(vcrypt_ctx *ctx, int cluster_size, size_t bytes_per_cta, int mode, int rounds, double *us_per_round,
-                       int *resident_clusters);
 
 #ifdef __cplusplus
 }

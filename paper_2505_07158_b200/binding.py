@@ -78,8 +78,6 @@ def lib() -> C.CDLL:
     L.vcrypt_frame_stats_device.argtypes = [_vp, _vp, C.c_size_t, C.POINTER(FrameStats), _vp, _vp]
     L.vcrypt_npcr_uaci_device.argtypes = [_vp, _vp, _vp, C.c_size_t, _vp, _vp, _vp]
     L.vcrypt_local_entropy_device.argtypes = [_vp, _vp, C.c_size_t, _vp, C.c_uint32, C.c_uint32, _vp, _vp]
-    L.vcrypt_memory_probe.argtypes = [_vp, C.c_int, C.c_size_t, C.c_int, C.POINTER(C.c_double)]
-    L.vcrypt_dsmem_probe.argtypes = [_vp, C.c_int, C.c_size_t, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     _lib = L
     return L
 
@@ -275,19 +273,6 @@ class Vcrypt:
                                                        xy.shape[0], side, out.ctypes.data, 0 if stream is None else int(stream)),
                     "vcrypt_local_entropy_device")
         return out
-
-    def memory_probe(self, which: int, frames: int, reps: int = 20) -> float:
-        """vcrypt_memory_probe: microseconds per repetition (0 sequential copy, 1 two-pass traffic, 2 column strips)."""
-        us = C.c_double()
-        self._check(self.L.vcrypt_memory_probe(self._p, which, frames, reps, C.byref(us)), "vcrypt_memory_probe")
-        return float(us.value)
-
-    def dsmem_probe(self, cluster_size: int, bytes_per_cta: int, mode: int, rounds: int = 20):
-        """vcrypt_dsmem_probe -> (microseconds per all-to-all round, resident clusters)."""
-        us, nc = C.c_double(), C.c_int()
-        self._check(self.L.vcrypt_dsmem_probe(self._p, cluster_size, bytes_per_cta, mode, rounds, C.byref(us), C.byref(nc)),
-                    "vcrypt_dsmem_probe")
-        return float(us.value), int(nc.value)
 
     def last_stage_ms(self):
         out = (C.c_double * 4)()

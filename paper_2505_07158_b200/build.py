@@ -22,7 +22,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 CXX_FLAGS = ["-O3", "-std=c++17", "-fPIC", "-ffp-contract=off", "-fno-fast-math", "-Wall", "-Wextra",
              "-fvisibility=hidden", f"-I{CUDA_HOME}/include"]
 # (source, extra flags); derive.cu holds the chaotic-map arithmetic: no FMA contraction
-CU_SOURCES = [("kernels.cu", []), ("cipher.cu", []), ("membench.cu", []), ("derive.cu", ["-fmad=false"]), ("sha256.cu", []), ("stats.cu", [])]
+CU_SOURCES = [("kernels.cu", []), ("cipher.cu", []), ("derive.cu", ["-fmad=false"]), ("sha256.cu", []), ("stats.cu", [])]
 # (source, extra flags)
 CXX_SOURCES = [
     ("vcrypt.cpp", []),

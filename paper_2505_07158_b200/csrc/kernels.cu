@@ -42,46 +42,9 @@
 #include <type_traits>
 
 #include "kernels.cuh"
+#include "ptx.cuh"
 
 namespace vk {
-
-// ---------------------------------------------------------------------------------------------
-// async-copy / mbarrier PTX (sm_90+; SASS: UBLKCP, UTMALDG, UTMAPF, SYNCS)
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
-    uint32_t ok;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-// Bounded wait: a copy that never lands must trap, not hang the GPU.
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-    for (uint32_t spin = 0; !mbar_try_wait(bar, parity); ++spin)
-        if (spin > (1u << 24)) __trap();
-}
-// shared -> global bulk copy
-__device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(__cvta_generic_to_global(gdst)),
-                 "r"(smem_u32(smem_src)), "r"(bytes)
-                 : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-}
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------------------------
 // Row pass: horizontal bit rotation (Algorithm 4 / Eq. 2 on the rows of Algorithm 3's bit matrix,
@@ -122,33 +85,6 @@ __device__ __forceinline__ uint2 row_param(const uint16_t *__restrict__ D, const
     return make_uint2((dw >> 2) << 4, ((plane_off + 4u * (dw & 3u)) << 8) | (sh & 31u));
 }
 
-// Programmatic dependent launch (PDL): a kernel launched with the programmatic-stream-serialization attribute may start
-// while its predecessor in the stream is still draining; pdl_wait() blocks until the predecessor has completed and its
-// writes are visible, pdl_trigger() lets the successor's CTAs be scheduled as soon as resources free up.
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-
-__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ uint64_t policy_evict_first() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-// global -> shared bulk copy (16-byte aligned, size a multiple of 16) with an L2 cache hint, completion on the mbarrier
-__device__ __forceinline__ void bulk_g2s_hint(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar, uint64_t pol) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
-            smem_u32(smem_dst)),
-        "l"(__cvta_generic_to_global(gsrc)), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_wait_read_0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-
 template <bool INV, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src, uint8_t *dst, const uint16_t *__restrict__ D,
                                                            Geom g, uint32_t nblocks, uint32_t NS, uint32_t NC) {
@@ -174,6 +110,7 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
         for (uint32_t s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
         mbar_init(ofull, 1);
         mbar_init(ofree, 1);
+        mbar_init_fence();
     }
     __syncthreads();
     pdl_wait();     // everything below reads or writes global memory the previous kernel of the stream may have written
@@ -357,29 +294,6 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
 constexpr int CE_PAD = 8;   // repeated strip rows
 constexpr int CE_G = 8;     // output rows per group
 
-__device__ __forceinline__ void tma_load_2d(void *smem_dst, const CUtensorMap *tm, int32_t x, int32_t y, uint64_t *bar,
-                                            uint64_t pol) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4}], [%2], %5;" ::
-            "r"(smem_u32(smem_dst)),
-        "l"(reinterpret_cast<uint64_t>(tm)), "r"(smem_u32(bar)), "r"(x), "r"(y), "l"(pol)
-        : "memory");
-}
-
-// L2 prefetch of one tensor tile (DRAM -> L2 only; no shared memory, no completion to wait for)
-__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap *tm, int32_t x, int32_t y) {
-    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(reinterpret_cast<uint64_t>(tm)), "r"(x),
-                 "r"(y)
-                 : "memory");
-}
-
-// p + off as one IMAD.WIDE.U32 (FMA pipe) instead of a two-instruction 64-bit add on the ALU pipe
-__device__ __forceinline__ uint64_t mad_wide_ptr(const void *p, uint32_t off) {
-    uint64_t r;
-    asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(r) : "r"(off), "l"(reinterpret_cast<uint64_t>(p)));
-    return r;
-}
-
 template <int X, int NT, int MINB, int DEPTH>
 __global__ void __launch_bounds__(NT, MINB)
     col_enc_kernel(const __grid_constant__ CUtensorMap tm_main, const __grid_constant__ CUtensorMap tm_pad,
@@ -407,6 +321,7 @@ __global__ void __launch_bounds__(NT, MINB)
         for (; pf_row < h && pf_row < CE_AHEAD + (DEPTH - 1) * GSTEP * CE_G; pf_row += pf_rows)
             tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
         mbar_init(bar, 1);
+        mbar_init_fence();
         pdl_wait();  // the strip is the row pass's output
         const uint64_t pol = policy_evict_first();
         mbar_expect_tx(bar, (h + CE_PAD) * X);
@@ -615,13 +530,18 @@ __global__ void __launch_bounds__(NT, MINB)
         for (; pf_row < h && pf_row < CD_AHEAD + (KD - 1) * 4u * GSTEP; pf_row += pf_rows)
             tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
         mbar_init(bar, 1);
+        mbar_init_fence();
         pdl_wait();  // the ciphertext may be the previous kernel's output
         const uint64_t pol = policy_evict_first();
         mbar_expect_tx(bar, h * X);
         const int32_t y0 = (int32_t)(f * h);
         for (uint32_t r0 = 0; r0 < h; r0 += box_rows) tma_load_2d(S + (size_t)r0 * X, &tm_src, (int32_t)x0, y0 + (int32_t)r0, bar, pol);
     }
-    // one thread per byte column of the strip: t = d_v mod h, the row offset of the column's source (D is an input)
+    // D and the keystream are inputs too: whoever wrote them (a kernel of the caller's, launched just before on this stream)
+    // must be complete before the first read -- only the L2 look-ahead above runs ahead of this wait
+    pdl_wait();
+    pdl_trigger();
+    // one thread per byte column of the strip: t = d_v mod h, the row offset of the column's source
     if (threadIdx.x >= NT - X) {
         const uint32_t xs = threadIdx.x - (NT - X);
         uint32_t x = x0 + xs;
@@ -630,8 +550,6 @@ __global__ void __launch_bounds__(NT, MINB)
         const uint32_t dv = D[(size_t)f * g.nD + c * (h + g.w) + h + jj];
         ups[xs] = (uint16_t)(dv - __umulhi(dv, h_magic) * h);  // d_v mod h  (h_magic = ceil(2^32 / h), d_v < 2^16)
     }
-    pdl_wait();
-    pdl_trigger();
 
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t sub = lane / LPS, j = lane % LPS;

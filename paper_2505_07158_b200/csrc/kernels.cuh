@@ -117,11 +117,4 @@ cudaError_t diff_device(const Geom &g, const uint8_t *d_a, const uint8_t *d_b, s
 cudaError_t block_hist_device(const Geom &g, const uint8_t *d_frames, size_t n, const uint32_t *d_xy, uint32_t k, uint32_t side,
                               uint32_t *d_bh, cudaStream_t st);
 
-// Memory-system probes (membench.cu): see vcrypt_memory_probe in include/vcrypt.h.
-cudaError_t memory_probe(const Geom &g, int which, size_t frames, int reps, cudaStream_t st, double *us_per_call);
-
-// Distributed-shared-memory exchange probe (membench.cu): see vcrypt_dsmem_probe in include/vcrypt.h.
-cudaError_t dsmem_probe(int cluster_size, size_t own_bytes, int mode, int rounds, double *us_per_round, int *max_active_clusters,
-                        int *clusters_launched);
-
 }  // namespace vk

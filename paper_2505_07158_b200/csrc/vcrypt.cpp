@@ -84,9 +84,6 @@ struct vcrypt_ctx {
     uint32_t *d_sched = nullptr;                  // kSchedSlots x cipher_sched_words(kSchedFrames), zero between launches
     cudaStream_t sched_owner[kSchedSlots] = {};
     int sched_n = 0;
-    // generic-path scratch for in-place calls
-    uint8_t *d_scratch = nullptr;
-    size_t scratch_bytes = 0;
     // bookkeeping
     uint64_t launches_last = 0, launches_total = 0;
     double stage_ms[4] = {0, 0, 0, 0};
@@ -116,6 +113,25 @@ int guarded(F &&body) noexcept {
         return VCRYPT_E_ARG;
     }
 }
+
+// Makes the context's device current for the duration of an entry point and puts the caller's device back afterwards.
+struct DeviceScope {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceScope(int dev) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+        else if (err == cudaSuccess) prev = -1;  // nothing to restore
+    }
+    ~DeviceScope() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+    DeviceScope(const DeviceScope &) = delete;
+    DeviceScope &operator=(const DeviceScope &) = delete;
+};
+#define VC_DEVICE(ctx)                            \
+    DeviceScope dev_scope__((ctx)->device);       \
+    if (dev_scope__.err != cudaSuccess) return cuda_fail((ctx), dev_scope__.err, "cudaSetDevice")
 
 bool is_pinned(const void *p) {
     cudaPointerAttributes a;
@@ -287,22 +303,21 @@ int launch_cipher(vcrypt_ctx *c, bool decrypt, const uint8_t *src, const uint16_
     } else {
         uint8_t *out = dst;
         const size_t bytes = n * c->g.frame_bytes;
-        if (dst == src) {  // the gather kernels cannot run in place: go through scratch
-            if (c->scratch_bytes < bytes) {
-                if (c->d_scratch) {
-                    VC_CUDA(c, cudaStreamSynchronize(st));
-                    VC_CUDA(c, cudaFree(c->d_scratch));
-                    c->d_scratch = nullptr;
-                    c->scratch_bytes = 0;
-                }
-                VC_CUDA(c, cudaMalloc(&c->d_scratch, bytes));
-                c->scratch_bytes = bytes;
-            }
-            out = c->d_scratch;
+        bool scratch = false;
+        if (dst == src) {  // the gather kernels cannot run in place: through a scratch buffer of this call, allocated and freed in
+                           // stream order (calls on other streams have their own)
+            void *tmp = nullptr;
+            VC_CUDA(c, cudaMallocAsync(&tmp, bytes, st));
+            out = static_cast<uint8_t *>(tmp);
+            scratch = true;
         }
         e = decrypt ? vk::decrypt_generic(c->g, src, D, B, n, out, st, &launches)
                     : vk::encrypt_generic(c->g, src, D, B, n, out, st, &launches);
         if (e == cudaSuccess && out != dst) e = cudaMemcpyAsync(dst, out, bytes, cudaMemcpyDeviceToDevice, st);
+        if (scratch) {
+            const cudaError_t ef = cudaFreeAsync(out, st);
+            if (e == cudaSuccess) e = ef;
+        }
     }
     c->launches_last += (uint64_t)launches;
     c->launches_total += (uint64_t)launches;
@@ -323,6 +338,7 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
     if (!(p->gamma >= -1.52 && p->gamma <= -0.06)) return VCRYPT_E_KEY;
     if (p->n_workers == 0 || p->width == 0 || p->height == 0) return VCRYPT_E_SHAPE;
     if (p->n_workers > (1u << 20) || p->width > (1u << 16) || p->height > (1u << 16)) return VCRYPT_E_SHAPE;
+    if ((uint64_t)3 * p->width * p->height >= ((uint64_t)1 << 31)) return VCRYPT_E_SHAPE;  // 32-bit byte offsets inside a frame
     vcrypt_ctx *c = new (std::nothrow) vcrypt_ctx;
     if (!c) return VCRYPT_E_NOMEM;
     int rc = VCRYPT_OK;
@@ -355,9 +371,9 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
         c->slices.resize(c->batch * (size_t)p->n_workers);
         c->subhash.resize(c->batch * (size_t)p->n_workers * 32u);
         if (rc == VCRYPT_OK && !(p->flags & VCRYPT_FLAG_HOST_ONLY)) {
-            int dev = p->device;
-            cudaError_t e = cudaSuccess;
-            if (dev < 0) e = cudaGetDevice(&dev);
+            int dev = p->device, prev_dev = -1;
+            cudaError_t e = cudaGetDevice(&prev_dev);
+            if (e == cudaSuccess && dev < 0) dev = prev_dev;
             if (e == cudaSuccess) e = cudaSetDevice(dev);
             if (e == cudaSuccess) e = vk::make_plan(c->g, dev, &c->plan);
             if (e == cudaSuccess) {
@@ -372,6 +388,7 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
                 c->device = dev;
                 c->slots.resize(p->n_streams ? p->n_streams : ((p->flags & VCRYPT_FLAG_DEVICE_HASH) ? 12 : 3));  // device hashing wants a deep pipeline (6 ms per band)
             }
+            if (prev_dev >= 0 && prev_dev != dev) cudaSetDevice(prev_dev);  // the caller's current device is left as it was
         }
     } catch (const std::bad_alloc &) {
         rc = VCRYPT_E_NOMEM;
@@ -389,7 +406,7 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
 extern "C" void vcrypt_destroy(vcrypt_ctx *c) {
     if (!c) return;
     if (c->cuda) {
-        cudaSetDevice(c->device);
+        DeviceScope scope(c->device);
         for (Slot &s : c->slots) free_slot(s);
         for (int i = 0; i + 1 < vcrypt_ctx::kPipeMax; ++i) {
             if (c->pipe_st[i]) { cudaStreamSynchronize(c->pipe_st[i]); cudaStreamDestroy(c->pipe_st[i]); }
@@ -399,10 +416,6 @@ extern "C" void vcrypt_destroy(vcrypt_ctx *c) {
         if (c->d_sched) {
             cudaDeviceSynchronize();
             cudaFree(c->d_sched);
-        }
-        if (c->d_scratch) {
-            cudaDeviceSynchronize();
-            cudaFree(c->d_scratch);
         }
     }
     delete c;
@@ -448,6 +461,8 @@ extern "C" int vcrypt_get_state(const vcrypt_ctx *c, double state_out[4], uint64
 extern "C" int vcrypt_set_state(vcrypt_ctx *c, const double state[4], uint64_t frames_done) {
     if (!c || !state) return VCRYPT_E_ARG;
     if (!vh::finite4(state)) return VCRYPT_E_STATE;
+    for (int k = 0; k < 4; ++k)
+        if (std::fabs(state[k]) >= 9007199254740992.0) return VCRYPT_E_STATE;  // 2^53, as for the key: integer parts stay exact
     std::memcpy(c->S, state, sizeof c->S);
     c->frames_done = frames_done;
     return VCRYPT_OK;
@@ -554,7 +569,7 @@ extern "C" int vcrypt_frame_hash_device(vcrypt_ctx *c, const void *d_frames, siz
         if (!c || !d_frames || !hashes_out || n == 0) return VCRYPT_E_ARG;
         if (!c->cuda) return VCRYPT_E_CUDA;
         if ((((uintptr_t)d_frames) & 15u) || c->g.row_bytes % 16u != 0) return VCRYPT_E_SHAPE;
-        VC_CUDA(c, cudaSetDevice(c->device));
+        VC_DEVICE(c);
         cudaStream_t st = static_cast<cudaStream_t>(stream);
         uint32_t *d_H = nullptr;
         cudaError_t e = cudaMalloc(&d_H, n * 32u);
@@ -572,7 +587,7 @@ extern "C" int vcrypt_derive_device(vcrypt_ctx *c, const uint8_t *hash, void *d_
         if (!c || !hash || !d_D || !d_B) return VCRYPT_E_ARG;
         if (!c->cuda) return VCRYPT_E_CUDA;
         if ((((uintptr_t)d_B) & 7u) || (((uintptr_t)d_D) & 1u)) return VCRYPT_E_ARG;
-        VC_CUDA(c, cudaSetDevice(c->device));
+        VC_DEVICE(c);
         cudaStream_t st = static_cast<cudaStream_t>(stream);
         const size_t irb = 2u * (size_t)c->p.n_workers * 4u * sizeof(double);
         double S[4];
@@ -616,7 +631,7 @@ static int device_call(vcrypt_ctx *c, bool decrypt, const void *d_in, const void
     uint8_t *o = static_cast<uint8_t *>(d_out);
     const size_t bytes = n * c->g.frame_bytes;
     if (a != o && a < o + bytes && o < a + bytes) return VCRYPT_E_ARG;  // partial overlap
-    VC_CUDA(c, cudaSetDevice(c->device));
+    VC_DEVICE(c);
     return launch_cipher(c, decrypt, a, static_cast<const uint16_t *>(d_D), static_cast<const uint8_t *>(d_B), n, o,
                          static_cast<cudaStream_t>(stream));
 }
@@ -657,7 +672,7 @@ extern "C" int vcrypt_frame_stats_device(vcrypt_ctx *c, const void *d_frames, si
     return guarded([&]() -> int {
         if (!c || !d_frames || !out || n == 0) return VCRYPT_E_ARG;
         if (!c->cuda) return VCRYPT_E_CUDA;
-        VC_CUDA(c, cudaSetDevice(c->device));
+        VC_DEVICE(c);
         cudaStream_t st = static_cast<cudaStream_t>(stream);
         uint32_t *d_hist = nullptr;
         unsigned long long *d_pairs = nullptr;
@@ -712,7 +727,7 @@ extern "C" int vcrypt_npcr_uaci_device(vcrypt_ctx *c, const void *d_a, const voi
     return guarded([&]() -> int {
         if (!c || !d_a || !d_b || !npcr || !uaci || n == 0) return VCRYPT_E_ARG;
         if (!c->cuda) return VCRYPT_E_CUDA;
-        VC_CUDA(c, cudaSetDevice(c->device));
+        VC_DEVICE(c);
         cudaStream_t st = static_cast<cudaStream_t>(stream);
         unsigned long long *d_out = nullptr;
         std::vector<unsigned long long> r(n * 6u);
@@ -746,7 +761,7 @@ extern "C" int vcrypt_local_entropy_device(vcrypt_ctx *c, const void *d_frames, 
         if (!c->cuda) return VCRYPT_E_CUDA;
         for (uint32_t b = 0; b < k; ++b)
             if ((uint64_t)xy[2 * b] + side > c->g.w || (uint64_t)xy[2 * b + 1] + side > c->g.h) return VCRYPT_E_ARG;
-        VC_CUDA(c, cudaSetDevice(c->device));
+        VC_DEVICE(c);
         cudaStream_t st = static_cast<cudaStream_t>(stream);
         uint32_t *d_xy = nullptr, *d_bh = nullptr;
         std::vector<uint32_t> bh(n * k * 768u);
@@ -770,34 +785,6 @@ extern "C" int vcrypt_local_entropy_device(vcrypt_ctx *c, const void *d_frames, 
     });
 }
 
-extern "C" int vcrypt_memory_probe(vcrypt_ctx *c, int which, size_t frames, int reps, double *us_per_rep) {
-    return guarded([&]() -> int {
-        if (!c || !us_per_rep || which < 0 || which > 2 || frames == 0 || reps < 1) return VCRYPT_E_ARG;
-        if (!c->cuda) return VCRYPT_E_CUDA;
-        VC_CUDA(c, cudaSetDevice(c->device));
-        const cudaError_t e = vk::memory_probe(c->g, which, frames, reps, nullptr, us_per_rep);
-        if (e == cudaErrorInvalidValue) return VCRYPT_E_ARG;
-        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return VCRYPT_E_NOMEM; }
-        if (e != cudaSuccess) return cuda_fail(c, e, "memory probe");
-        return VCRYPT_OK;
-    });
-}
-
-extern "C" int vcrypt_dsmem_probe(vcrypt_ctx *c, int cluster_size, size_t bytes_per_cta, int mode, int rounds, double *us_per_round,
-                                  int *resident_clusters) {
-    return guarded([&]() -> int {
-        if (!c || !us_per_round) return VCRYPT_E_ARG;
-        if (!c->cuda) return VCRYPT_E_CUDA;
-        VC_CUDA(c, cudaSetDevice(c->device));
-        int maxc = 0, launched = 0;
-        const cudaError_t e = vk::dsmem_probe(cluster_size, bytes_per_cta, mode, rounds, us_per_round, &maxc, &launched);
-        if (resident_clusters) *resident_clusters = launched;
-        if (e == cudaErrorInvalidValue) { cudaGetLastError(); return VCRYPT_E_ARG; }
-        if (e != cudaSuccess) return cuda_fail(c, e, "dsmem probe");
-        return VCRYPT_OK;
-    });
-}
-
 // =====================================================================================================
 // host-buffer pipeline: Algorithm 1's loop over frames, batched and overlapped
 // =====================================================================================================
@@ -808,7 +795,7 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
     c->launches_last = 0;
     for (double &v : c->stage_ms) v = 0.0;
     if (n == 0) return VCRYPT_OK;
-    VC_CUDA(c, cudaSetDevice(c->device));
+    VC_DEVICE(c);
     const size_t fb = c->g.frame_bytes, nD = c->g.nD;
     const bool in_pinned = is_pinned(in) && is_pinned(in + n * fb - 1);
     const bool out_pinned = is_pinned(out) && is_pinned(out + n * fb - 1);

@@ -139,3 +139,35 @@ def digest(a: np.ndarray) -> str:
     """SHA-256 of the generated bytes (logged so a numpy stream change cannot
     silently alter a run); hashlib here is bookkeeping, not the method."""
     return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
+
+
+# ------------------------------------------------------------------------------------------------------
+# channel damage applied to CIPHERTEXT before decryption (PAPER.md:547-557, Fig. 8 - 9: cropping, salt-and-pepper and
+# Gaussian noise).  Inputs of the robustness harness only: no cipher arithmetic here.  The paper's figure gives no noise
+# levels; DESIGN.md states the ones used (densities 0.01 / 0.05 / 0.1 per byte, Gaussian variances 0.001 / 0.01 of full scale).
+# ------------------------------------------------------------------------------------------------------
+def salt_and_pepper(cipher: np.ndarray, density: float, seed: int) -> np.ndarray:
+    """A copy of `cipher` in which a fraction `density` of the bytes is forced to 0 or 255 (equal odds)."""
+    rng = np.random.default_rng(seed)
+    out = cipher.copy()
+    hit = rng.random(cipher.shape) < density
+    salt = rng.random(cipher.shape) < 0.5
+    out[hit & salt] = 255
+    out[hit & ~salt] = 0
+    return out
+
+
+def gaussian_noise(cipher: np.ndarray, variance: float, seed: int) -> np.ndarray:
+    """A copy of `cipher` with additive zero-mean Gaussian noise of the given variance (full scale = 1), rounded and clipped."""
+    rng = np.random.default_rng(seed)
+    noisy = cipher.astype(np.float64) + rng.normal(0.0, 255.0 * np.sqrt(variance), cipher.shape)
+    return np.clip(np.rint(noisy), 0, 255).astype(np.uint8)
+
+
+def crop(cipher: np.ndarray, fraction: float) -> np.ndarray:
+    """A copy of `cipher` whose top-left rectangle covering `fraction` of the frame area is blanked (Fig. 8)."""
+    out = cipher.copy()
+    h, w = cipher.shape[-3], cipher.shape[-2]
+    s = float(np.sqrt(fraction))
+    out[..., : int(round(h * s)), : int(round(w * s)), :] = 0
+    return out

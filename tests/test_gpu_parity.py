@@ -5,8 +5,8 @@ Kernel level  : vcrypt_encrypt_device / vcrypt_decrypt_device with random D, B (
                 oracle's literal bit-matrix Algorithms 3-7, over tiled shapes, ragged any-shape cases, special
                 distances and in-place calls.
 Whole path    : vcrypt_encrypt_frames / vcrypt_decrypt_frames (rows a1-a12) against the oracle's Algorithm 1
-                on the BASELINE.json configs: C1, C2 in full element by element; C3-C5 at full size in bench's
-                launch configuration with every hash compared, sampled frames compared element by element
+                on the BASELINE.json configs, every frame element by element: C1, C2 in full; C3 all 30 frames,
+                C4 100 frames, C5 20 frames at full size in bench's launch configuration, with every hash compared
                 and the round trip checked on every frame.
 """
 import numpy as np
@@ -113,6 +113,41 @@ def test_in_place_and_forced_generic(torch_cuda, vb, orc, w, h, nf, generic):
     assert np.array_equal(run_device(torch_cuda, v, F, D, B), ref)
     assert np.array_equal(run_device(torch_cuda, v, F, D, B, inplace=True), ref)
     assert np.array_equal(run_device(torch_cuda, v, ref, D, B, decrypt=True, inplace=True), F)
+
+
+@pytest.mark.parametrize("w,h,nf", [(256, 256, 1), (64, 48, 3), (112, 20, 3), (64, 16, 5), (2048, 24, 1), (144, 1028, 1), (640, 480, 7),
+                                    (64, 48, 40), (720, 480, 2), (1920, 1080, 3)])
+@pytest.mark.parametrize("tune", [(0, 0, 0, 0), (1, 1, 1, 3), (2, 7, 2, 1)])
+def test_persistent_kernel_matches_oracle(torch_cuda, vb, orc, w, h, nf, tune):
+    """VCRYPT_FLAG_PERSISTENT: the whole call as ONE persistent kernel (row team + strip team per SM, work by ticket, per-frame
+    counters between the passes; cipher.cu) -- the same bytes as the oracle in both directions and in place, whatever the
+    tuning (row stages, blocks per ticket, window, keystream ring), over strips with a ragged end, a half row group at the
+    bottom, more frames than the window, and 40 frames of a tiny shape (many tickets per CTA)."""
+    F, D, B = rnd_case(w, h, nf, seed=w + h + nf)
+    v = gpu_ctx(vb, w, h, flags=vb.FLAG_PERSISTENT, tune=tune)
+    want = oracle_frames(orc, F, D, B)
+    E = run_device(torch_cuda, v, F, D, B)
+    assert v.launch_count()[0] == 1
+    assert np.array_equal(E, want)
+    assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
+    assert np.array_equal(run_device(torch_cuda, v, F, D, B, inplace=True), want)
+    assert np.array_equal(run_device(torch_cuda, v, want, D, B, decrypt=True, inplace=True), F)
+    # the launch state is left clean: the same context again, other data
+    F2, D2, B2 = rnd_case(w, h, nf, seed=w + h + nf + 1)
+    assert np.array_equal(run_device(torch_cuda, v, F2, D2, B2), oracle_frames(orc, F2, D2, B2))
+
+
+def test_persistent_kernel_whole_path(vb, orc):
+    """vcrypt_encrypt_frames / vcrypt_decrypt_frames with VCRYPT_FLAG_PERSISTENT on config 2 (batches over the slots' streams,
+    one launch state per stream): every frame against the oracle."""
+    cfg = synth.CONFIGS["C2"]
+    frames = synth.video(cfg)
+    enc = gpu_ctx(vb, cfg.w, cfg.h, batch=5, n_streams=3, flags=vb.FLAG_PERSISTENT)
+    C, Hs = enc.encrypt_frames(frames)
+    Co, Ho = oracle_clip(orc, "C2", cfg.frames)
+    assert np.array_equal(C, Co) and np.array_equal(Hs, Ho)
+    dec = gpu_ctx(vb, cfg.w, cfg.h, batch=7, n_streams=2, flags=vb.FLAG_PERSISTENT)
+    assert np.array_equal(dec.decrypt_frames(C, Hs), frames)
 
 
 # NEXT-4 (SURVEY 8(f)): the other resolutions of the paper's Tab. VIII (PAPER.md:563-572): 360 x 240 takes the any-shape
@@ -256,8 +291,8 @@ def test_device_call_argument_errors(torch_cuda, vb):
 @pytest.mark.parametrize("cfgname,nf,pairs_enc,pairs_dec", [("C4", 30, 6, 5), ("C5", 8, 8, 4)])
 def test_full_size_resident_clip_as_bench_times_it(torch_cuda, vb, orc, cfgname, nf, pairs_enc, pairs_dec):
     """The launch configuration bench.py's kernel leg times -- ONE *_device call on a resident clip with the default schedule
-    (FHD: launch pairs of 5 frames when encrypting, 6 when decrypting; 4K: 1 and 2) -- at full frame size, sampled frames
-    against the oracle, every frame through the inverse."""
+    (FHD: launch pairs of 5 frames when encrypting, 6 when decrypting; 4K: 1 and 2) -- at full frame size, every frame
+    against the oracle and through the inverse."""
     torch = torch_cuda
     cfg = synth.CONFIGS[cfgname]
     w, h = cfg.w, cfg.h
@@ -269,8 +304,9 @@ def test_full_size_resident_clip_as_bench_times_it(torch_cuda, vb, orc, cfgname,
     v.encrypt_device(dF, dD, dB, dE)
     torch.cuda.synchronize()
     assert v.launch_count()[0] == 2 * pairs_enc
-    for k in sorted({0, nf // 2 - 1, nf // 2, nf - 1}):
-        assert np.array_equal(dE[k].cpu().numpy(), orc.confuse_xor(F[k], D[k], B[k])), k
+    E = dE.cpu().numpy()
+    for k in range(nf):  # every frame against the oracle
+        assert np.array_equal(E[k], orc.confuse_xor(F[k], D[k], B[k])), k
     dP = torch.empty_like(dF)
     v.decrypt_device(dE, dD, dB, dP)
     torch.cuda.synchronize()
@@ -316,9 +352,9 @@ def test_config2_full(vb, orc):
     assert np.array_equal(P, frames)
 
 
-def sampled_parity(vb, orc, cfg, nframes, sample, pinned):
-    """Full-size config in bench's launch configuration: all hashes, sampled frames element by element
-    (oracle D, B follow the whole chain), round trip on every frame."""
+def full_parity(vb, orc, cfg, nframes, pinned):
+    """Full-size config in bench's launch configuration: every hash and every frame's ciphertext element by element
+    against the oracle (its D, B follow the whole chain), round trip on every frame."""
     import torch
 
     if pinned:
@@ -337,8 +373,7 @@ def sampled_parity(vb, orc, cfg, nframes, sample, pinned):
         H = orc.frame_hash(frames[k], synth.N_WORKERS)
         assert H == Hs[k].tobytes(), k
         D, B = oc.derive(H)
-        if k in sample:
-            assert np.array_equal(C[k], orc.confuse_xor(frames[k], D, B)), k
+        assert np.array_equal(C[k], orc.confuse_xor(frames[k], D, B)), k
     dec = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
     P = dec.decrypt_frames(C, Hs)
     assert np.array_equal(P, frames)
@@ -347,18 +382,18 @@ def sampled_parity(vb, orc, cfg, nframes, sample, pinned):
 
 def test_config3_fhd_batch1(vb, orc):
     cfg = synth.CONFIGS["C3"]
-    sampled_parity(vb, orc, cfg, cfg.frames, {0, 1, 2, 15, 29}, pinned=False)
+    full_parity(vb, orc, cfg, cfg.frames, pinned=False)  # all 30 frames
 
 
 def test_config4_fhd_batches_of_8_three_streams(vb, orc):
     cfg = synth.CONFIGS["C4"]
-    enc = sampled_parity(vb, orc, cfg, 100, {0, 7, 8, 9, 50, 95, 96, 99}, pinned=True)  # 12 full batches + 4
+    enc = full_parity(vb, orc, cfg, 100, pinned=True)  # 12 full batches + 4, all 100 frames against the oracle
     assert enc.launch_count()[1] >= 13
 
 
 def test_config5_4k(vb, orc):
     cfg = synth.CONFIGS["C5"]
-    sampled_parity(vb, orc, cfg, 20, {0, 7, 8, 19}, pinned=True)
+    full_parity(vb, orc, cfg, 20, pinned=True)  # all 20 frames
 
 
 def test_config4_one_bit_pairs_npcr_uaci(vb, torch_cuda):
@@ -443,6 +478,18 @@ def test_device_hashing_rejects_unaligned_rows(torch_cuda, vb):
     assert v.L.vcrypt_frame_hash_device(v._p, F.data_ptr(), 1, out.ctypes.data, 0) == vb.E_SHAPE
 
 
+_oracle_clips = {}
+
+
+def oracle_clip(orc, cfgname, nframes):
+    """The oracle's ciphertext and hashes of the first frames of a config's clip (computed once per module run)."""
+    key = (cfgname, nframes)
+    if key not in _oracle_clips:
+        cfg = synth.CONFIGS[cfgname]
+        _oracle_clips[key] = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h).encrypt_frames(synth.video(cfg, nframes))
+    return _oracle_clips[key]
+
+
 @pytest.mark.parametrize("flags", ["derive", "hash", "both"])
 @pytest.mark.parametrize("cfgname,nframes", [("C1", 1), ("C2", 24), ("C4", 20)])
 def test_whole_path_with_device_derivation(vb, orc, cfgname, nframes, flags):
@@ -456,39 +503,11 @@ def test_whole_path_with_device_derivation(vb, orc, cfgname, nframes, flags):
     ref = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
     C2, H2 = ref.encrypt_frames(frames)
     assert np.array_equal(Hs, H2) and np.array_equal(C, C2)
-    oc = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
-    k = min(2, nframes)
-    Co, Ho = oc.encrypt_frames(frames[:k])
-    assert np.array_equal(C[:k], Co) and np.array_equal(Hs[:k], Ho)
+    Co, Ho = oracle_clip(orc, cfgname, nframes)  # every frame against the oracle
+    assert np.array_equal(C, Co) and np.array_equal(Hs, Ho)
     dec = gpu_ctx(vb, cfg.w, cfg.h, batch=3, n_streams=2, flags=fl)
     assert np.array_equal(dec.decrypt_frames(C, Hs), frames)
     assert enc.get_state()[1] == nframes and np.array_equal(enc.get_state()[0], ref.get_state()[0])
-
-
-def test_memory_probe_hook(vb):
-    """vcrypt_memory_probe (bench hook): plausible times, argument errors."""
-    import ctypes as C
-
-    v = gpu_ctx(vb, 640, 480)
-    t_copy, t_two, t_strip = (v.memory_probe(k, 24, 5) for k in (0, 1, 2))
-    assert 0.5 < t_copy < 1000 and 0.5 < t_strip < 1000
-    assert t_two > t_copy  # five trips through L2 against two
-    us = C.c_double()
-    assert v.L.vcrypt_memory_probe(v._p, 3, 1, 1, C.byref(us)) == vb.E_ARG
-    assert v.L.vcrypt_memory_probe(v._p, 0, 0, 1, C.byref(us)) == vb.E_ARG
-    assert v.L.vcrypt_memory_probe(v._p, 0, 1, 0, C.byref(us)) == vb.E_ARG
-    assert v.L.vcrypt_memory_probe(v._p, 0, 1, 1, None) == vb.E_ARG
-
-
-def test_dsmem_probe_hook(vb):
-    """Design hook: an all-to-all between the CTAs of a cluster through distributed shared memory runs and is timed."""
-    v = gpu_ctx(vb, 256, 256)
-    for cs, own, mode in ((2, 32 * 1024, 0), (8, 64 * 1024, 1), (16, 64 * 1024, 0)):
-        us, nc = v.dsmem_probe(cs, own, mode, 4)
-        assert us > 0 and nc >= 1
-    for cs, own, mode in ((0, 65536, 0), (17, 65536, 0), (8, 65536, 2), (8, 1000, 0), (8, 200 * 1024, 0)):
-        with pytest.raises(vb.VcryptError):
-            v.dsmem_probe(cs, own, mode, 4)
 
 
 def test_failed_call_leaves_chain_untouched(vb):

@@ -59,7 +59,7 @@ def test_frame_stats_match_oracle(torch_cuda, vb, kind, w, h, nf):
                 if np.isnan(ref):
                     assert np.isnan(r["corr"][f, c, d])
                 else:
-                    assert np.isclose(r["corr"][f, c, d], ref, rtol=1e-7, atol=1e-9), (c, d)
+                    assert np.isclose(r["corr"][f, c, d], ref, rtol=RTOL, atol=1e-9), (c, d)
 
 
 @pytest.mark.parametrize("w,h,nf", [(64, 48, 2), (17, 9, 2), (1, 1, 1), (640, 480, 1)])

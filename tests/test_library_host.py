@@ -59,6 +59,8 @@ def test_strerror_and_describe():
     (dict(gamma=-0.05), vb.E_KEY), (dict(gamma=-1.53), vb.E_KEY), (dict(gamma=float("nan")), vb.E_KEY),
     (dict(key=(float("inf"), 1, 1, 1)), vb.E_KEY), (dict(key=(1e300, 1, 1, 1)), vb.E_KEY),
     (dict(n=0), vb.E_SHAPE), (dict(w=0), vb.E_SHAPE), (dict(h=0), vb.E_SHAPE), (dict(w=70000), vb.E_SHAPE),
+    (dict(w=32768, h=32768), vb.E_SHAPE),  # 3wh >= 2^31: byte offsets inside a frame are 32-bit in the kernels
+    (dict(w=26752, h=26756), vb.E_SHAPE),  # just above 2^31 / 3 pixels
 ])
 def test_init_rejects_bad_parameters(bad, code):
     kw = dict(key=synth.KEY, gamma=synth.GAMMA, n=4, w=16, h=8)
@@ -82,15 +84,6 @@ def test_null_arguments_and_host_only_gpu_calls():
     assert L.vcrypt_encrypt_frames(v._p, buf.ctypes.data, 1, buf.ctypes.data, hs.ctypes.data) == vb.E_CUDA
     assert L.vcrypt_decrypt_frames(v._p, buf.ctypes.data, hs.ctypes.data, 1, buf.ctypes.data) == vb.E_CUDA
     assert L.vcrypt_encrypt_device(v._p, C.c_void_p(256), C.c_void_p(256), C.c_void_p(256), 1, C.c_void_p(256), None) == vb.E_CUDA
-
-
-def test_memory_probe_needs_a_gpu_context():
-    import ctypes as C
-
-    v = host_ctx(64, 48, 4)
-    us = C.c_double()
-    assert v.L.vcrypt_memory_probe(v._p, 0, 1, 1, C.byref(us)) == vb.E_CUDA
-    assert v.L.vcrypt_memory_probe(None, 0, 1, 1, C.byref(us)) == vb.E_ARG
 
 
 def test_init_without_gpu_fails_loudly():
@@ -169,6 +162,10 @@ def test_state_checkpoint_resume():
     with pytest.raises(vb.VcryptError) as ei:
         c.set_state([float("nan"), 0, 0, 0], 0)
     assert ei.value.code == vb.E_STATE
+    with pytest.raises(vb.VcryptError) as ei:  # same bound as the key: |v| < 2^53, so that the integer part stays exact
+        c.set_state([2.0 ** 53, 0, 0, 0], 0)
+    assert ei.value.code == vb.E_STATE
+    c.set_state([2.0 ** 53 - 1, 0, 0, 0], 0)
 
 
 def test_production_sha256_fips_vectors():
