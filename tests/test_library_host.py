@@ -60,7 +60,7 @@ def test_strerror_and_describe():
     (dict(key=(float("inf"), 1, 1, 1)), vb.E_KEY), (dict(key=(1e300, 1, 1, 1)), vb.E_KEY),
     (dict(n=0), vb.E_SHAPE), (dict(w=0), vb.E_SHAPE), (dict(h=0), vb.E_SHAPE), (dict(w=70000), vb.E_SHAPE),
     (dict(w=32768, h=32768), vb.E_SHAPE),  # 3wh >= 2^31: byte offsets inside a frame are 32-bit in the kernels
-    (dict(w=26752, h=26756), vb.E_SHAPE),  # just above 2^31 / 3 pixels
+    (dict(w=26760, h=26760), vb.E_SHAPE),  # just above 2^31 / 3 pixels
 ])
 def test_init_rejects_bad_parameters(bad, code):
     kw = dict(key=synth.KEY, gamma=synth.GAMMA, n=4, w=16, h=8)
