@@ -36,11 +36,25 @@ from paper_2505_07158_b200 import parallel, synth  # noqa: E402
 METRIC = "FHD frames/s encrypted"
 UNIT = "frames/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum of the two kernels of one launch pair (5 FHD frames: row pass 30.9 + 2.9 MB,
-# column pass 27.0 + 3.2 MB), from the ncu --set full capture summarised in profiles/r1n_ncu_full_summary.csv; below the
-# 93.4 MB of algorithmic bytes of a pair because most of its output is still dirty in L2 when the kernel ends
-NCU_TRAFFIC_PER_CALL = {"C4": 64.0e6}
-NCU_COL_SHARE = 0.544  # column pass's share of a launch pair's serialised time in the same capture (19.6 of 36.1 us)
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ALL kernels of one kernel-only step of this script, per launch
+# pair, from an ncu pass over `bench.py --kernel-leg-only` in the step's own configuration: one row per config, written by
+# hand from the capture named in profiles/r2_README.md
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
+
+
+def ncu_traffic(cfg_name, frames_per_pair):
+    """-> (DRAM bytes per launch pair, column pass's share of a pair's serialised time) for this config, or (None, None)."""
+    try:
+        import csv
+
+        with open(TRAFFIC_FILE) as f:
+            for row in csv.DictReader(f):
+                if row["config"] == cfg_name:
+                    per_frame = (float(row["dram_read_bytes_per_step"]) + float(row["dram_write_bytes_per_step"])) / float(row["frames_per_step"])
+                    return per_frame * frames_per_pair, float(row["column_pass_time_share"])
+    except Exception:
+        pass
+    return None, None
 
 
 def hbm_peak():
@@ -138,6 +152,184 @@ def workload_name(cfg):
             f"key = 4 doubles, n_workers = {synth.N_WORKERS}")
 
 
+def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, hold_ms=50.0):
+    """Kernel-only timing on a resident clip: encrypt as ONE call (the library's resident-clip schedule), encrypt as one call
+    per batch of cfg.batch frames on one stream (config 4 as BASELINE.json words it), decrypt as one call.  CUDA events on
+    the calling stream.  Returns a dict; the ciphertext is left in d_E."""
+    import time as _t
+
+    kctx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams,
+                     host_threads=1, device=torch.cuda.current_device(), flags=args.kernel_flags)
+    stream = torch.cuda.current_stream().cuda_stream
+    d_E = torch.empty_like(d_F)
+    out = {}
+
+    def clip_step():
+        kctx.encrypt_device(d_F, d_D, d_B, d_E, stream)
+        return kctx.launch_count()[0]
+
+    def batch_step():
+        n = 0
+        for b0 in range(0, T, cfg.batch):
+            b1 = min(T, b0 + cfg.batch)
+            kctx.encrypt_device(d_F[b0:b1], d_D[b0:b1], d_B[b0:b1], d_E[b0:b1], stream)
+            n += kctx.launch_count()[0]
+        return n
+
+    # W untimed steps, held for at least hold_ms of GPU work: the timed steps must not see the clock ramp of a GPU that idled
+    # during the host-side set-up (a kernel-only step lasts about a millisecond)
+    warm_steps, t_warm = 0, _t.perf_counter()
+    while warm_steps < W or (_t.perf_counter() - t_warm < hold_ms * 1e-3 and warm_steps < 2000):
+        clip_step()
+        warm_steps += 1
+        if warm_steps >= W:
+            torch.cuda.synchronize()
+    barrier()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    launches = 0
+    ev[0].record()
+    for k in range(K):
+        launches += clip_step()
+        ev[k + 1].record()
+    barrier()
+    out["step_ms"] = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
+    out["total_ms"] = ev[0].elapsed_time(ev[K])
+    out["launches"] = launches
+    out["warm_steps"] = warm_steps
+    out["digest_first2"] = synth.digest(d_E[:2].cpu().numpy())
+    out["digest_all"] = synth.digest(d_E.cpu().numpy())
+
+    KB = max(1, min(K, 5))
+    d_E.zero_()
+    for _ in range(2):
+        batch_step()
+    barrier()
+    bv = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    bv[0].record()
+    bl = 0
+    for _ in range(KB):
+        bl += batch_step()
+    bv[1].record()
+    barrier()
+    out["batches_ms_frame"] = bv[0].elapsed_time(bv[1]) / KB / T
+    out["batches_steps"] = KB
+    out["batches_launches_per_step"] = bl // KB
+    out["batches_same"] = bool(synth.digest(d_E.cpu().numpy()) == out["digest_all"])
+
+    d_P = torch.empty_like(d_F)
+    for _ in range(2):
+        kctx.decrypt_device(d_E, d_D, d_B, d_P, stream)
+    barrier()
+    dv = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    dv[0].record()
+    for _ in range(KB):
+        kctx.decrypt_device(d_E, d_D, d_B, d_P, stream)
+    dv[1].record()
+    barrier()
+    out["dec_ms_frame"] = dv[0].elapsed_time(dv[1]) / KB / T
+    out["dec_steps"] = KB
+    out["decrypt_ok"] = bool(torch.equal(d_P, d_F))
+    out["d_E"] = d_E
+    kctx.destroy()
+    return out
+
+
+def c5_leg(vb, torch, peak, frames=40, steps=3):
+    """Bounded 4K leg (config 5's shape, a resident clip of `frames` frames with random D, B: the kernels' time does not depend
+    on the values): kernel-only encrypt and decrypt as one call each, checked by the round trip and one frame against the oracle."""
+    cfg = synth.CONFIGS["C5"]
+    g = torch.Generator(device="cuda")
+    g.manual_seed(5)
+    F = torch.randint(0, 256, (frames, cfg.h, cfg.w, 3), dtype=torch.uint8, device="cuda", generator=g)
+    B = torch.randint(0, 256, (frames, cfg.h, cfg.w, 3), dtype=torch.uint8, device="cuda", generator=g)
+    D = torch.randint(-32768, 32767, (frames, 3 * (cfg.h + cfg.w)), dtype=torch.int16, device="cuda", generator=g)
+    E, P = torch.empty_like(F), torch.empty_like(F)
+    v = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, host_threads=1, device=torch.cuda.current_device())
+    alg = 9 * cfg.w * cfg.h + 6 * (cfg.w + cfg.h)
+    res = {"workload": f"C5 shape {cfg.w}x{cfg.h}x3, resident clip of {frames} frames, one call per direction, random D and B", "steps": steps}
+    for name, fn, src, dst in (("encrypt", v.encrypt_device, F, E), ("decrypt", v.decrypt_device, E, P)):
+        for _ in range(3):
+            fn(src, D, B, dst)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            fn(src, D, B, dst)
+        e1.record()
+        torch.cuda.synchronize()
+        us = 1e3 * e0.elapsed_time(e1) / steps / frames
+        res[name] = {"us_per_frame": us, "frames_per_s": 1e6 / us, "frac": alg / (us * 1e-6) / 1e9 / peak}
+    O = oracle_lib()
+    k = frames // 2
+    res["roundtrip_ok"] = bool(torch.equal(P, F))
+    res["frame_vs_oracle_ok"] = bool(np.array_equal(E[k].cpu().numpy(), O.confuse_xor(F[k].cpu().numpy(), D[k].cpu().numpy().view(np.uint16), B[k].cpu().numpy())))
+    traffic, _ = ncu_traffic("C5", 1.0)
+    res["traffic_per_frame"] = traffic
+    v.destroy()
+    return res
+
+
+def c3_latency_leg(vb, torch, threads, frames=30):
+    """Config 3: one FHD frame per call (batch 1), host-side hashing and derivation, pinned buffers: per-frame latency end to
+    end and the paper's delay rate (share of frames that take longer than 1000 ms / frame rate; 30 FPS here)."""
+    cfg = synth.CONFIGS["C3"]
+    h_in = torch.empty((frames, cfg.h, cfg.w, 3), dtype=torch.uint8).pin_memory()
+    synth.video(cfg, min(frames, 8), out=h_in.numpy())
+    for t in range(8, frames):
+        h_in[t].copy_(h_in[t % 8])
+        h_in[t, 0, 0, 0] = t
+    h_out = torch.empty_like(h_in).pin_memory()
+    hh = torch.empty((frames, 32), dtype=torch.uint8)
+    v = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=1, n_streams=cfg.n_streams, host_threads=threads,
+                  device=torch.cuda.current_device())
+    for t in range(3):  # warm-up: buffers, streams
+        v.encrypt_frames(h_in[t:t + 1], h_out[t:t + 1], hh[t:t + 1])
+    v.destroy()
+    v = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=1, n_streams=cfg.n_streams, host_threads=threads,
+                  device=torch.cuda.current_device())
+    v.encrypt_frames(h_in[:1], h_out[:1], hh[:1])
+    v.set_state(vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, flags=vb.FLAG_HOST_ONLY).get_state()[0], 0)
+    ms = []
+    for t in range(frames):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        v.encrypt_frames(h_in[t:t + 1], h_out[t:t + 1], hh[t:t + 1])
+        ms.append(1e3 * (time.perf_counter() - t0))
+    O = oracle_lib()
+    oc = O.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    C_or, H_or = oc.encrypt_frames(h_in.numpy()[:2])
+    ok = bool(np.array_equal(C_or, h_out.numpy()[:2]) and np.array_equal(H_or, hh.numpy()[:2]))
+    v.destroy()
+    limit = 1000.0 / 30.0
+    return {"workload": f"C3: {cfg.w}x{cfg.h}x3, {frames} frames, one frame per vcrypt_encrypt_frames call, hashing and derivation on {threads} host threads",
+            "ms_per_frame_median": statistics.median(ms), "ms_per_frame_max": max(ms), "ms_per_frame_mean": statistics.fmean(ms),
+            "delay_rate_30fps": sum(1 for x in ms if x > limit) / len(ms), "frames_vs_oracle": 2, "ok": ok}
+
+
+def pcie_ceiling(torch, h_in, h_out, batch, reps=3):
+    """What the box's PCIe link gives the end-to-end leg: the same pinned buffers moved with plain cudaMemcpyAsync, one copy per
+    batch each way, uploads and downloads on two streams at the same time, no kernels.  -> (seconds per clip, H2D GB/s, D2H GB/s)."""
+    T = h_in.shape[0]
+    d_a = torch.empty((batch,) + tuple(h_in.shape[1:]), dtype=torch.uint8, device="cuda")
+    d_b = torch.empty_like(d_a)
+    s_up, s_dn = torch.cuda.Stream(), torch.cuda.Stream()
+    best = None
+    for _ in range(reps + 1):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for b0 in range(0, T, batch):
+            b1 = min(T, b0 + batch)
+            with torch.cuda.stream(s_up):
+                d_a[: b1 - b0].copy_(h_in[b0:b1], non_blocking=True)
+            with torch.cuda.stream(s_dn):
+                h_out[b0:b1].copy_(d_b[: b1 - b0], non_blocking=True)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        best = dt if best is None or dt < best else best
+    nbytes = h_in.numel()
+    return best, nbytes / best / 1e9, nbytes / best / 1e9
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -147,6 +339,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--frames", type=int, default=0, help="frames per step (default: the config's clip length)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra-legs", action="store_true", help="skip the bounded C5 (4K) and C3 (single-frame latency) legs")
+    ap.add_argument("--kernel-leg-only", action="store_true",
+                    help="only the kernel-only legs, exactly --warmup untimed steps: the command profiles/ captures under ncu")
+    ap.add_argument("--persistent", action="store_true", help="kernel-only legs through the persistent kernel (VCRYPT_FLAG_PERSISTENT)")
     ap.add_argument("--derive", default="auto", choices=["auto", "host", "device"],
                     help="where the worker systems (D, B) of the end-to-end leg run: host lanes or the GPU (same bytes)")
     ap.add_argument("--hash", default="auto", choices=["auto", "host", "device"],
@@ -169,6 +365,7 @@ def main():
 
     from paper_2505_07158_b200 import binding as vb
 
+    args.kernel_flags = vb.FLAG_PERSISTENT if args.persistent else 0
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -183,6 +380,12 @@ def main():
     fb, nD = 3 * cfg.w * cfg.h, 3 * (cfg.w + cfg.h)
     ncores = os.cpu_count() or 1
     threads = max(1, ncores // world)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
 
     # ---- inputs: rank r gets its own clip (seed + r) in pinned host memory --------------------------------
     rcfg = parallel.rank_clip_config(cfg, rank, T)
@@ -203,111 +406,44 @@ def main():
     B_all = torch.empty((T, cfg.h, cfg.w, 3), dtype=torch.uint8).pin_memory()
     for t in range(T):
         ctx.derive(ctx.frame_hash(frames_np[t]), D_all[t], B_all.numpy()[t])
+    ctx.destroy()
     d_F = h_in.cuda(non_blocking=True)
     d_B = B_all.cuda(non_blocking=True)
     d_D = torch.from_numpy(D_all.view(np.int16)).cuda()
-    d_E = torch.empty_like(d_F)
     torch.cuda.synchronize()
     del B_all
-    kctx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams,
-                     host_threads=threads, device=local)
-    stream = torch.cuda.current_stream().cuda_stream
 
-    def kernel_step():
-        # one call on the resident clip: the library cuts it into launch pairs (row pass + column pass) of about 31 MB of
-        # frames and alternates them over two streams forked from / joined into `stream` (vcrypt_params.pipe_*)
-        kctx.encrypt_device(d_F, d_D, d_B, d_E, stream)
-        return kctx.launch_count()[0]
-
-    def kernel_step_batches():
-        # context figure: one call per batch of cfg.batch frames, every launch on `stream` (the schedule before pipe_*)
-        for b0 in range(0, T, cfg.batch):
-            b1 = min(T, b0 + cfg.batch)
-            kctx.encrypt_device(d_F[b0:b1], d_D[b0:b1], d_B[b0:b1], d_E[b0:b1], stream)
-
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    # ---- kernel-only: CUDA events on the launching stream -----------------------------------------------
-    # W untimed steps; a kernel-only step lasts about a millisecond, so the warm-up is also held for at least 50 ms of GPU
-    # work: the timed steps must not see the clock ramp of a GPU that idled during the host-side set-up.  (Measured: 3 steps
-    # or 50 ms of warm-up -> 0.600 - 0.604 of the copy rate; 250 ms of warm-up -> 0.594 with sw_power_cap reported: the
-    # timed region of 10 steps is 14 ms, a burst like the copy the peak was measured with.)
-    warm_steps, t_warm = 0, time.perf_counter()
-    while warm_steps < W or (time.perf_counter() - t_warm < 0.05 and warm_steps < 2000):
-        kernel_step()
-        warm_steps += 1
-        if warm_steps >= W:
-            torch.cuda.synchronize()
-    barrier()
+    # ---- kernel-only legs: CUDA events on the launching stream ---------------------------------------------
     sampler = ClockSampler(local) if rank == 0 else None
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
-    launches = 0
-    ev[0].record()
-    for k in range(K):
-        launches += kernel_step()
-        ev[k + 1].record()
-    barrier()
-    step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
-    kern_ms_total = ev[0].elapsed_time(ev[K])
-    kernel_out_digest = synth.digest(d_E[:2].cpu().numpy())
-    kernel_all_digest = synth.digest(d_E.cpu().numpy())
-    pairs_per_step = max(1, launches // (2 * K))
-
-    # ---- context figure: the same frames in calls of cfg.batch frames on one stream ----------------------------------
-    KB = max(1, min(K, 5))
-    d_E.zero_()
-    for _ in range(2):
-        kernel_step_batches()
-    barrier()
-    bv = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    bv[0].record()
-    for _ in range(KB):
-        kernel_step_batches()
-    bv[1].record()
-    barrier()
-    batches_ms_frame = bv[0].elapsed_time(bv[1]) / KB / T
-    batches_same = bool(synth.digest(d_E.cpu().numpy()) == kernel_all_digest)
-
-    # ---- context figures: the inverse kernels on the same clip, and what the memory system allows for these bytes ----
-    def decrypt_step():
-        kctx.decrypt_device(d_E, d_D, d_B, d_P, stream)
-
-    d_P = torch.empty_like(d_F)
-    for _ in range(2):
-        decrypt_step()
-    barrier()
-    dv = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    KD = max(1, min(K, 5))
-    dv[0].record()
-    for _ in range(KD):
-        decrypt_step()
-    dv[1].record()
-    barrier()
-    dec_ms_frame = dv[0].elapsed_time(dv[1]) / KD / T
-    decrypt_ok = bool(torch.equal(d_P, d_F))
-    del d_P
-    probes = {}
-    if rank == 0:
-        nb = min(cfg.batch, T)
-        for which, name in ((0, "sequential_copy"), (1, "two_pass_traffic_sequential"), (2, "column_strips_read_write")):
-            probes[name] = kctx.memory_probe(which, nb, 20) / nb  # us per frame
+    kl = kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, hold_ms=0.0 if args.kernel_leg_only else 50.0)
+    kern_ms_total = kl["total_ms"]
+    pairs_per_step = max(1, kl["launches"] // (2 * K)) if not args.persistent else max(1, kl["launches"] // K)
+    if args.kernel_leg_only:
+        if rank == 0:
+            print(json.dumps({"kernel_leg_only": True, "config": cfg.name, "frames_per_step": T, "steps": K, "warmup_steps_run": kl["warm_steps"],
+                              "us_per_frame": 1e3 * kern_ms_total / K / T, "launches_per_step": kl["launches"] // K,
+                              "batches_us_per_frame": 1e3 * kl["batches_ms_frame"], "decrypt_us_per_frame": 1e3 * kl["dec_ms_frame"],
+                              "ok": kl["batches_same"] and kl["decrypt_ok"]}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    del kl["d_E"]
 
     # pipeline depth of the end-to-end leg: the config's 3 streams with host hashing; device hashing (6 ms per band on a
     # GPU thread) needs a deeper pipeline to be hidden (results do not depend on it)
     e2e_streams = args.e2e_streams or (12 if args.hash == "device" else cfg.n_streams)
+    e2e_batch = args.e2e_batch or cfg.batch
+    e2e_flags = (vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0) | (vb.FLAG_DEVICE_HASH if args.hash == "device" else 0)
+
+    def e2e_ctx(flags=e2e_flags):
+        return vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=e2e_batch, n_streams=e2e_streams,
+                         host_threads=threads, device=local, flags=flags, device_hash_bands=args.hash_bands)
+
     # ---- end to end through the host-buffer call -----------------------------------------------------------
-    ectx = None
+    ectx = e2e_ctx()
     e2e_s = []
+    n_first = min(16, T)
     for k in range(W + K):
-        ectx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=args.e2e_batch or cfg.batch,
-                         n_streams=e2e_streams, host_threads=threads, device=local,
-                         flags=(vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0) |
-                         (vb.FLAG_DEVICE_HASH if args.hash == "device" else 0),
-                         device_hash_bands=args.hash_bands) if ectx is None else ectx
         if k == W:
             barrier()
             t_e2e0 = time.perf_counter()
@@ -316,25 +452,23 @@ def main():
         if k >= W:
             e2e_s.append(time.perf_counter() - t0)
         if k == 0:
-            first_out = h_out[:2].numpy().copy()
-            first_hash = h_hash[:2].numpy().copy()
+            first_out = h_out[:n_first].numpy().copy()
+            first_hash = h_hash[:n_first].numpy().copy()
             first_all_digest = synth.digest(h_out.numpy())
     barrier()
     e2e_total = time.perf_counter() - t_e2e0
     stage = ectx.last_stage_ms()
+    ectx.destroy()
     clocks = sampler.stop() if sampler else None
 
-    # ---- context: the receiver's side end to end (vcrypt_decrypt_frames: no hashing, H is transmitted) -----------------------
+    # ---- context: what the PCIe link alone gives these buffers, and the receiver's side end to end ---------
+    pcie_s, pcie_up, pcie_dn = pcie_ceiling(torch, h_in, h_out, e2e_batch) if rank == 0 else (None, None, None)
     h_plain = torch.empty_like(h_in).pin_memory()
-    fresh = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=args.e2e_batch or cfg.batch, n_streams=e2e_streams,
-                      host_threads=threads, device=local, flags=(vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0) |
-                      (vb.FLAG_DEVICE_HASH if args.hash == "device" else 0), device_hash_bands=args.hash_bands)
+    fresh = e2e_ctx()
     fresh.encrypt_frames(h_in, h_out, h_hash)  # the clip from the start of the chain (the timed calls carried the chain on)
     fresh.destroy()
     dec_s = []
-    dctx = vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=args.e2e_batch or cfg.batch,
-                     n_streams=e2e_streams, host_threads=threads, device=local,
-                     flags=vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0)
+    dctx = e2e_ctx(vb.FLAG_DEVICE_DERIVE if args.derive == "device" else 0)
     state0 = dctx.get_state()[0].copy()
     for k in range(4):  # the first call allocates the pipeline's buffers: not timed
         dctx.set_state(state0, 0)  # back to the start of the chain (checkpoint / resume hook)
@@ -354,73 +488,102 @@ def main():
             dist.destroy_process_group()
         return
 
+    peak, peak_src = hbm_peak()
+    # ---- bounded extra legs (rank 0): 4K kernels, single-frame latency -----------------------------------------------
+    del d_F, d_B, d_D
+    torch.cuda.empty_cache()
+    c5 = c3 = None
+    if not args.no_extra_legs and cfg.name == "C4":
+        c5 = c5_leg(vb, torch, peak)
+        torch.cuda.empty_cache()
+        c3 = c3_latency_leg(vb, torch, threads)
+
     # ---- no number for a wrong result: first pass of the e2e path (fresh chain) against the oracle -----------
-    check = {"frames_vs_oracle": 2}
-    cpu_baseline = None
     n_or = {"C1": 1, "C2": 24, "C3": 16, "C4": 16, "C5": 4}[cfg.name]
-    n_or = min(n_or, T) if not args.no_cpu_baseline else min(2, T)
+    n_or = min(n_or, T, n_first) if not args.no_cpu_baseline else min(2, T)
     fps_or, C_or, H_or = time_oracle(cfg, frames_np, n_or)
-    m = min(2, n_or)
-    check["e2e_vs_oracle"] = bool(np.array_equal(C_or[:m], first_out[:m]) and np.array_equal(H_or[:m], first_hash[:m]))
-    check["kernels_vs_e2e_first_frames"] = bool(kernel_out_digest == synth.digest(first_out))
-    check["kernels_vs_e2e_all_frames"] = bool(kernel_all_digest == first_all_digest)
-    check["kernels_in_batches_same_bytes"] = batches_same
-    check["decrypt_kernels_invert"] = decrypt_ok
+    check = {"frames_vs_oracle": n_or}
+    check["e2e_vs_oracle"] = bool(np.array_equal(C_or, first_out[:n_or]) and np.array_equal(H_or, first_hash[:n_or]))
+    check["kernels_vs_e2e_first_frames"] = bool(kl["digest_first2"] == synth.digest(first_out[:2]))
+    check["kernels_vs_e2e_all_frames"] = bool(kl["digest_all"] == first_all_digest)
+    check["kernels_in_batches_same_bytes"] = kl["batches_same"]
+    check["decrypt_kernels_invert"] = kl["decrypt_ok"]
     check["e2e_decrypt_returns_clip"] = e2e_decrypt_ok
+    if c5:
+        check["c5_roundtrip_and_oracle_frame"] = bool(c5["roundtrip_ok"] and c5["frame_vs_oracle_ok"])
+    if c3:
+        check["c3_vs_oracle"] = c3["ok"]
     ok = all(v for k, v in check.items() if k != "frames_vs_oracle")
     check["ok"] = bool(ok)
     if not ok:
         print(json.dumps({"metric": METRIC, "error": "GPU output does not match the oracle", "check": check}))
         raise SystemExit(1)
+    cpu_baseline = None
     if not args.no_cpu_baseline:
         cpu_baseline = {"value": fps_or, "unit": UNIT, "cores": 1, "kind": "oracle",
                         "sample": f"first {n_or} frames of the clip, oracle/vcrypt_oracle.c single-threaded, "
                                   f"{ncores} host cores present"}
 
-    peak, peak_src = hbm_peak()
     alg_bytes_frame = 3 * fb + 2 * nD  # read F_o + read B + write F_e + read D (~9wh)
     value = parallel.whole_job_rate(world, T, K, kern_ms_total * 1e-3)
     achieved = alg_bytes_frame * T * K / (kern_ms_total * 1e-3) / 1e9
     e2e_value = parallel.whole_job_rate(world, T, K, e2e_total)
+    frames_per_pair = T / pairs_per_step
+    traffic, col_share = ncu_traffic(cfg.name, frames_per_pair)
+    batches_frac = alg_bytes_frame / (kl["batches_ms_frame"] * 1e-3) / 1e9 / peak
+    dec_frac = alg_bytes_frame / (kl["dec_ms_frame"] * 1e-3) / 1e9 / peak
+    kernel_name = ("cipher_kernel (persistent: row team + strip team per SM)" if args.persistent else
+                   "row_pass_kernel<false> + col_enc_kernel<64> = one launch pair of vcrypt_encrypt_device (col_enc_kernel is the larger "
+                   f"share{'' if col_share is None else f', {col_share:.0%} of a pair in profiles/'})")
+    pcie_fps = world * T / pcie_s if pcie_s else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": kern_ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u8", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "frames_per_step": T, "ms_per_frame_kernel": kern_ms_total / K / T,
                    "l2": f"inputs larger than L2: {3 * fb * T / 1e6:.0f} MB streamed per step, no flush needed",
-                   "host_threads": threads, "host_cores": ncores, "warmup_steps_run": warm_steps, "describe": vb.describe()},
+                   "host_threads": threads, "host_cores": ncores, "warmup_steps_run": kl["warm_steps"], "describe": vb.describe()},
+        # config 4 exactly as BASELINE.json words it (batches of 8 frames per launch pair, every launch on ONE stream), and the
+        # headline against the nominal 8 TB/s the north star quotes: neither is hidden inside `roofline`
+        "c4_batches_of_8_one_stream": {"value": 1e3 / kl["batches_ms_frame"], "unit": UNIT, "us_per_frame": 1e3 * kl["batches_ms_frame"],
+                                       "frac": batches_frac, "frac_of_8TBs_nominal": batches_frac * peak / 8000.0},
+        "frac_of_8TBs_nominal": achieved / 8000.0,
+        "targets": {"kernel_60pct_of_8TBs_nominal": {"met": bool(achieved / 8000.0 >= 0.6), "frac": achieved / 8000.0},
+                    "kernel_60pct_of_measured_copy_rate": {"met": bool(achieved / peak >= 0.6), "frac": achieved / peak},
+                    "e2e_1000_frames_per_s": {"met": bool(e2e_value >= 1000.0), "value": e2e_value},
+                    "bit_exact": {"met": True}},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": T * ((fb + 64 * synth.N_WORKERS) if args.derive == "device" else (2 * fb + 2 * nD)),
                 "d2h_bytes_per_step": T * fb,
                 "ms_per_frame": 1e3 * e2e_total / (K * T), "ms_per_step_median": 1e3 * statistics.median(e2e_s),
-                "stage_ms_last_call": stage, "derive": args.derive, "hash": args.hash, "hash_bands_on_gpu": (args.hash_bands or synth.N_WORKERS) if args.hash == "device" else 0, "batch": args.e2e_batch or cfg.batch, "n_streams": e2e_streams,
+                "stage_ms_last_call": stage, "derive": args.derive, "hash": args.hash,
+                "hash_bands_on_gpu": (args.hash_bands or synth.N_WORKERS) if args.hash == "device" else 0, "batch": e2e_batch, "n_streams": e2e_streams,
+                # the same pinned buffers through plain cudaMemcpyAsync, one copy per batch each way, both directions at once
+                "pcie_copy_only": {"frames_per_s": pcie_fps, "h2d_gbs": pcie_up, "d2h_gbs": pcie_dn},
+                "frac_of_pcie": (e2e_value / pcie_fps) if pcie_fps else None,
                 "timer": "wall clock around vcrypt_encrypt_frames, pinned host in/out"},
-        "gpu_launches": launches,
+        "gpu_launches": kl["launches"],
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC_PER_CALL.get(cfg.name),
-                     "kernel": "row_pass_kernel<false> + col_enc_kernel<64> = one launch pair of vcrypt_encrypt_device "
-                               f"(col_enc_kernel is the larger share, {NCU_COL_SHARE:.0%} in profiles/); the step is ONE call on the "
-                               f"resident clip = {pairs_per_step} launch pairs alternating over 2 streams, so achieved = the step's "
-                               "algorithmic bytes / its duration (CUDA events on the calling stream, which the internal stream "
-                               "forks from and joins); single_stream_batches = the same frames as one call per batch on one stream",
+                     "traffic": traffic,
+                     "traffic_source": "profiles/r2_dram_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum over all kernels of one step of "
+                                       "`bench.py --kernel-leg-only` under ncu, per launch pair",
+                     "kernel": kernel_name + f"; the step is ONE call on the resident clip = {pairs_per_step} launch pairs alternating over 2 "
+                               "streams, so achieved = the step's algorithmic bytes / its duration (CUDA events on the calling stream, which the "
+                               "internal stream forks from and joins)",
                      "algorithmic_bytes_per_frame": alg_bytes_frame,
                      "launch_pairs_per_step": pairs_per_step,
-                     "frames_per_launch_pair": T / pairs_per_step,
-                     "algorithmic_bytes_per_launch_pair": alg_bytes_frame * T / pairs_per_step,
+                     "frames_per_launch_pair": frames_per_pair,
+                     "algorithmic_bytes_per_launch_pair": alg_bytes_frame * frames_per_pair,
                      "us_per_launch_pair": 1e3 * kern_ms_total / K / pairs_per_step,
-                     "single_stream_batches": {"frames_per_call": min(cfg.batch, T), "us_per_frame": 1e3 * batches_ms_frame,
-                                               "us_per_call": 1e3 * batches_ms_frame * min(cfg.batch, T),
-                                               "frac": alg_bytes_frame / (batches_ms_frame * 1e-3) / 1e9 / peak, "steps": KB},
+                     "single_stream_batches": {"frames_per_call": min(cfg.batch, T), "us_per_frame": 1e3 * kl["batches_ms_frame"],
+                                               "us_per_call": 1e3 * kl["batches_ms_frame"] * min(cfg.batch, T),
+                                               "frac": batches_frac, "steps": kl["batches_steps"]},
                      "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
-                     "step_ms_median": statistics.median(step_ms), "step_ms_min": min(step_ms),
-                     # what the memory system allows for the same bytes (vcrypt_memory_probe, us per frame): a plain
-                     # copy, the 5-trips-through-L2 traffic of any two-pass design, the column pass's strided DRAM side
-                     "memory_probes_us_per_frame": probes,
-                     "two_pass_ceiling_frac": (alg_bytes_frame / (probes["two_pass_traffic_sequential"] * 1e-6) / 1e9 / peak)
-                     if probes.get("two_pass_traffic_sequential") else None},
+                     "step_ms_median": statistics.median(kl["step_ms"]), "step_ms_min": min(kl["step_ms"])},
         "e2e_decrypt": {"value": world * T / min(dec_s), "unit": UNIT, "ms_per_frame": 1e3 * min(dec_s) / T,
                         "note": "vcrypt_decrypt_frames from the start of the chain, best of 3 after one warm-up call, pinned host in/out, rank 0's time"},
-        "decrypt_kernels": {"value": 1e3 / dec_ms_frame, "unit": UNIT, "us_per_frame": 1e3 * dec_ms_frame,
-                            "frac": alg_bytes_frame / (dec_ms_frame * 1e-3) / 1e9 / peak, "steps": KD},
+        "decrypt_kernels": {"value": 1e3 / kl["dec_ms_frame"], "unit": UNIT, "us_per_frame": 1e3 * kl["dec_ms_frame"],
+                            "frac": dec_frac, "steps": kl["dec_steps"]},
+        "c5_4k_kernels": c5, "c3_single_frame_latency": c3,
         "cpu_baseline": cpu_baseline, "clocks": clocks, "check": check,
         "context": {"paper_ms_per_fhd_frame": 25.84, "paper_hw": "Xeon Gold 6226R + RTX 3090 (PAPER.md:5, :568); not a target"},
     }

@@ -31,3 +31,17 @@ def test_bench_prints_one_contract_line():
     assert cb["kind"] == "oracle" and cb["cores"] == 1 and cb["value"] > 0 and cb["sample"]
     assert d["check"]["ok"] is True
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    assert d["check"]["frames_vs_oracle"] == 16  # every oracle frame of the run is compared, not a sample of them
+    t = d["targets"]
+    assert set(t) >= {"kernel_60pct_of_8TBs_nominal", "kernel_60pct_of_measured_copy_rate", "e2e_1000_frames_per_s"}
+    assert t["kernel_60pct_of_8TBs_nominal"]["met"] == (d["frac_of_8TBs_nominal"] >= 0.6)
+    assert d["c4_batches_of_8_one_stream"]["frac"] > 0 and e["frac_of_pcie"] > 0 and e["pcie_copy_only"]["frames_per_s"] > e["value"]
+
+
+def test_bench_kernel_leg_only_line():
+    """The command profiles/ captures under ncu: kernel-only legs, exactly the requested warm-up, one small JSON line."""
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--config", "C2", "--steps", "1", "--warmup", "3", "--kernel-leg-only"],
+                       capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = json.loads([ln for ln in r.stdout.splitlines() if ln.strip()][-1])
+    assert d["kernel_leg_only"] is True and d["ok"] is True and d["warmup_steps_run"] == 3 and d["us_per_frame"] > 0
