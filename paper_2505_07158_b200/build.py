@@ -29,8 +29,8 @@ CXX_SOURCES = [
     ("host_sha256.cpp", []),
     ("host_derive.cpp", []),
     ("host_lhcs_scalar.cpp", []),
-    ("host_lhcs_avx2.cpp", ["-mavx2"]),
-    ("host_lhcs_avx512.cpp", ["-mavx512f", "-mavx512dq", "-mprefer-vector-width=512"]),
+    ("host_lhcs_avx2.cpp", ["-mavx2", "-mclflushopt"]),
+    ("host_lhcs_avx512.cpp", ["-mavx512f", "-mavx512dq", "-mprefer-vector-width=512", "-mclflushopt"]),
 ]
 HEADERS = ["host.hpp", "kernels.cuh", "ptx.cuh", "thread_pool.hpp", "host_lhcs_lanes.inc", os.path.join("..", "..", "include", "vcrypt.h")]
 

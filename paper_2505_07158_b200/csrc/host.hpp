@@ -40,6 +40,7 @@ struct WorkerSlice {
     size_t nd;
     uint8_t *B;       // slice of the frame's B
     size_t nb;
+    bool flush_B;     // write the slice's cache lines back once it is complete (it goes to the GPU next, see host_lhcs_lanes.inc)
 };
 
 // Derives `count` workers (any count; lanes are padded internally).  isa: 0 scalar, 1 AVX2 (4 lanes),

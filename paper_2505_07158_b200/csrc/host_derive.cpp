@@ -94,6 +94,7 @@ void make_slices(const double *IR, uint32_t n, uint32_t w, uint32_t h, uint16_t 
         s.nd = d1 - d0;
         s.B = B + b0;
         s.nb = b1 - b0;
+        s.flush_B = false;
     }
 }
 

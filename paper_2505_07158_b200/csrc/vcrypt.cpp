@@ -511,7 +511,7 @@ void hash_frames(vcrypt_ctx *c, const uint8_t *frames, size_t m, uint8_t *hashes
 
 // D and B of m frames whose hashes are known, written frame after frame into D / B.  S is advanced.
 // Returns VCRYPT_E_STATE if a chaotic state became non-finite.
-int derive_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, uint16_t *D, uint8_t *B) {
+int derive_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, uint16_t *D, uint8_t *B, bool flush_B = false) {
     const uint32_t n = c->p.n_workers;
     const double gamma = c->p.gamma;
     // the chain is serial in the frame index, and cheap (2n * K_m RK4 steps per frame)
@@ -520,6 +520,10 @@ int derive_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, u
         if (!vh::chain_step(S, gamma, n, hashes + 32u * f, IR)) return VCRYPT_E_STATE;
         vh::make_slices(IR, n, c->g.w, c->g.h, D + f * c->g.nD, B + f * c->g.frame_bytes, c->slices.data() + f * n);
     }
+    // a batch whose keystream would stay in the cores' private caches (single-frame calls: latency) is flushed by the jobs
+    // that write it; a large batch spills to memory by itself and the flushes would only cost the host-bound pipeline time
+    if (flush_B && m * c->g.frame_bytes <= ((size_t)32 << 20))
+        for (size_t i = 0; i < m * n; ++i) c->slices[i].flush_B = true;
     const int isa = c->isa;
     const size_t lanes = isa == 2 ? 8 : isa == 1 ? 4 : 1;
     const size_t groups = (n + lanes - 1) / lanes;
@@ -868,7 +872,7 @@ static int run_frames(vcrypt_ctx *c, bool decrypt, const uint8_t *in, const uint
         }
         {  // steps 7-14
             const auto t0 = clk::now();
-            const int r = dev_derive ? chain_frames(c, S, hs, m, s.h_IR) : derive_frames(c, S, hs, m, s.h_D, s.h_B);
+            const int r = dev_derive ? chain_frames(c, S, hs, m, s.h_IR) : derive_frames(c, S, hs, m, s.h_D, s.h_B, true);
             c->stage_ms[1] += ms_since(t0);
             if (r != VCRYPT_OK) return r;
         }
