@@ -90,7 +90,7 @@ typedef struct vcrypt_params {
     /* tuning of the persistent cipher kernel (0 -> chosen from the frame size); none of them affects results */
     uint32_t tune_row_stages;      /* input stages of the row team's shared-memory ring                            */
     uint32_t tune_row_item_blocks; /* blocks of 4 rows per row ticket                                              */
-    uint32_t tune_window;          /* frames the leading pass may run ahead of the following one (0 -> 4)          */
+    uint32_t tune_window;          /* frames the leading pass may run ahead of the following one (0 -> 8)          */
     uint32_t tune_ring;            /* chunks of the strip team's keystream ring in shared memory (1, 2; 3: none)   */
 } vcrypt_params;
 
