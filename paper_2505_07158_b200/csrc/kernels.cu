@@ -856,12 +856,33 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
             p.row_nc = nc;
             p.row_big = row_big;
             p.smem_row = row_smem_bytes(g, ns);
+            // Decrypt direction: where three CTAs with one input stage each fit an SM, the inverse row pass runs as three small
+            // CTAs (160 compute threads: the pass waits on its copies, not on its arithmetic -- 128 to 480 compute threads give
+            // the same time) instead of two with two stages.  Its CTAs then share an SM with the decrypt column pass's (three per
+            // SM, the same 70 KB) in any mix.  Measured at FHD: decrypt 5.42 -> 5.19 us per frame (batches of 8: 6.50 -> 6.21);
+            // the encrypt direction, whose column pass runs two CTAs per SM, loses with it (4.41 -> 4.60) and keeps two.
+            p.row_nc_dec = nc;
+            p.row_ns_dec = ns;
+            p.smem_row_dec = p.smem_row;
+            if (!row_big && 3 * (p.smem_row + 1024) > (size_t)smem_sm && 3 * (row_smem_bytes(g, 1) + 1024) <= (size_t)smem_sm) {
+                p.row_nc_dec = nc < 160 ? nc : 160;
+                p.row_ns_dec = 1;
+                p.smem_row_dec = row_smem_bytes(g, 1);
+            }
             int rc = (int)((size_t)smem_sm / (p.smem_row + 1024));
             const int by_threads = 2048 / (nc + 32);
             if (rc > by_threads) rc = by_threads;
             if (rc > 3) rc = 3;
             if (rc < 1 || row_big) rc = 1;
             p.row_grid_max = rc * sms;
+            {
+                int rd = (int)((size_t)smem_sm / (p.smem_row_dec + 1024));
+                const int bt = 2048 / (p.row_nc_dec + 32);
+                if (rd > bt) rd = bt;
+                if (rd > 3) rd = 3;
+                if (rd < 1 || row_big) rd = 1;
+                p.row_grid_max_dec = rd * sms;
+            }
             // frames per launch pair: the intermediate of one pair should mostly fit the 126 MB L2.  Measured (profiles/):
             // 100 MB beats 56 MB (4K: 25.1 vs 27.4 us per frame; fewer, longer launches), and even a fully spilled
             // intermediate costs little -- the L2 trips bound the path, not the DRAM.
@@ -877,6 +898,7 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
             if (e != cudaSuccess) return e;
             e = cudaFuncSetAttribute(row_pass_kernel<false, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
             if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
+            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_dec);
             if (!e) e = cudaFuncSetAttribute(row_pass_kernel<false, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
             if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
             if (e != cudaSuccess) return e;
@@ -910,15 +932,16 @@ static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, 
     // persistent CTAs, balanced: the fewest rounds the resident CTAs allow, then the smallest grid that needs no more rounds
     // (FHD, 5 frames: 1350 blocks = 5 rounds of 270 CTAs instead of 296 CTAs of which 166 take a 5th block; measured 4.50 ->
     // 4.44 us per frame, decrypt 5.58 -> 5.46: no CTA idles through a last round while it holds its share of the SM)
-    const uint32_t gmax = (uint32_t)p.row_grid_max;
+    const bool small = INV && p.row_ns_dec == 1 && p.row_nc_dec + 32 <= 256 && !p.row_big;  // three small CTAs per SM (decrypt)
+    const uint32_t gmax = (uint32_t)(INV ? p.row_grid_max_dec : p.row_grid_max);
     const uint32_t rounds = (nblocks + gmax - 1u) / gmax;
     const uint32_t grid = (nblocks + rounds - 1u) / rounds;
-    const uint32_t nt = (uint32_t)p.row_nc + 32u;
-    if (p.row_big)
-        return launch_pdl(row_pass_kernel<INV, 1024, 1>, grid, nt, p.smem_row, st, src, dst, D, g, nblocks, (uint32_t)p.row_ns,
-                          (uint32_t)p.row_nc);
-    return launch_pdl(row_pass_kernel<INV, 512, 2>, grid, nt, p.smem_row, st, src, dst, D, g, nblocks, (uint32_t)p.row_ns,
-                      (uint32_t)p.row_nc);
+    const uint32_t nc = (uint32_t)(INV ? p.row_nc_dec : p.row_nc), ns = (uint32_t)(INV ? p.row_ns_dec : p.row_ns);
+    const size_t smem = INV ? p.smem_row_dec : p.smem_row;
+    const uint32_t nt = nc + 32u;
+    if (p.row_big) return launch_pdl(row_pass_kernel<INV, 1024, 1>, grid, nt, smem, st, src, dst, D, g, nblocks, ns, nc);
+    if (small) return launch_pdl(row_pass_kernel<true, 256, 3>, grid, nt, smem, st, src, dst, D, g, nblocks, ns, nc);
+    return launch_pdl(row_pass_kernel<INV, 512, 2>, grid, nt, smem, st, src, dst, D, g, nblocks, ns, nc);
 }
 
 // tensor map of an n*h x 3w byte matrix with tiles of X bytes x `rows` rows

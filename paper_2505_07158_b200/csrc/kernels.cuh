@@ -30,6 +30,8 @@ struct Plan {
     int row_ns;            // row pass: stages of the shared-memory ring
     bool row_big;          // row pass: one CTA of up to 1024 threads per SM (wide frames)
     int row_grid_max;      // row pass: persistent CTAs (resident CTAs per SM x SMs)
+    int row_nc_dec, row_ns_dec, row_grid_max_dec;  // the same for the inverse row pass (decrypt): three small CTAs per SM where they fit
+    size_t smem_row_dec;
     uint32_t box_rows;     // column pass: rows per TMA tensor tile (largest divisor of h that is <= 256)
     uint32_t h_magic;      // ceil(2^32 / h): d mod h without a division for d < 2^16
     void *encode_tiled;    // cuTensorMapEncodeTiled, resolved through the runtime (no link-time libcuda dependency)

@@ -351,7 +351,7 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
             // bytes of frames per launch pair, to the nearest frame.  Measured on B200 with two streams (us per frame, 300-frame
             // FHD clip, pairs of 4 / 5 / 6): encrypt 4.77 / 4.70 / 4.79, decrypt 5.65 / 5.68 / 5.56; 640x480 best at 30-40 frames,
             // 4K at 1: two pairs in flight keep their intermediates in L2
-            const size_t target[2] = {(size_t)31 << 20, (size_t)37 << 20};  // encrypt, decrypt
+            const size_t target[2] = {(size_t)31 << 20, (size_t)31 << 20};  // encrypt, decrypt (decrypt with three small row-pass CTAs per SM: pairs of 4 / 5 / 6 / 7 FHD frames 5.22 / 5.14 / 5.31 / 5.42 us per frame)
             for (int d = 0; d < 2; ++d) {
                 const size_t pf = p->pipe_frames ? p->pipe_frames : (target[d] + c->g.frame_bytes / 2) / c->g.frame_bytes;
                 c->pipe_frames[d] = pf < 1 ? 1 : pf;

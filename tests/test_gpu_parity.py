@@ -288,10 +288,10 @@ def test_device_call_argument_errors(torch_cuda, vb):
     assert L.vcrypt_encrypt_device(v._p, dF.data_ptr(), dD.data_ptr(), dB.data_ptr(), 0, dF.data_ptr(), st) == vb.OK
 
 
-@pytest.mark.parametrize("cfgname,nf,pairs_enc,pairs_dec", [("C4", 30, 6, 5), ("C5", 8, 8, 4)])
+@pytest.mark.parametrize("cfgname,nf,pairs_enc,pairs_dec", [("C4", 30, 6, 6), ("C5", 8, 8, 8)])
 def test_full_size_resident_clip_as_bench_times_it(torch_cuda, vb, orc, cfgname, nf, pairs_enc, pairs_dec):
     """The launch configuration bench.py's kernel leg times -- ONE *_device call on a resident clip with the default schedule
-    (FHD: launch pairs of 5 frames when encrypting, 6 when decrypting; 4K: 1 and 2) -- at full frame size, every frame
+    (FHD: launch pairs of 5 frames; 4K: 1) -- at full frame size, every frame
     against the oracle and through the inverse."""
     torch = torch_cuda
     cfg = synth.CONFIGS[cfgname]
