@@ -137,6 +137,19 @@ def test_persistent_kernel_matches_oracle(torch_cuda, vb, orc, w, h, nf, tune):
     assert np.array_equal(run_device(torch_cuda, v, F2, D2, B2), oracle_frames(orc, F2, D2, B2))
 
 
+def test_persistent_kernel_4k_narrow_strips(torch_cuda, vb, orc):
+    """At 3840 x 2160 a 64-byte strip leaves no room for the row team: the persistent kernel takes 32-byte strips (eight
+    sub-warps per warp), one row stage, no keystream ring.  Two frames against the oracle, and back."""
+    w, h, nf = 3840, 2160, 2
+    F, D, B = rnd_case(w, h, nf, seed=99)
+    v = gpu_ctx(vb, w, h, flags=vb.FLAG_PERSISTENT)
+    E = run_device(torch_cuda, v, F, D, B)
+    assert v.launch_count()[0] == 1
+    for k in range(nf):
+        assert np.array_equal(E[k], orc.confuse_xor(F[k], D[k], B[k])), k
+    assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
+
+
 def test_persistent_kernel_whole_path(vb, orc):
     """vcrypt_encrypt_frames / vcrypt_decrypt_frames with VCRYPT_FLAG_PERSISTENT on config 2 (batches over the slots' streams,
     one launch state per stream): every frame against the oracle."""
