@@ -61,6 +61,8 @@ extern "C" {
 #define VCRYPT_FLAG_DEVICE_DERIVE 8u  /* worker systems -> D, B on the GPU (same bytes): the host only
                                          hashes and runs the serial LHCS_m chain; D and B never cross PCIe */
 #define VCRYPT_FLAG_PERSISTENT 32u    /* one persistent kernel per call (cipher.cu: row team + strip team per SM) instead of the row-pass / column-pass kernel pairs */
+#define VCRYPT_FLAG_ROW_TMA 64u       /* row pass through TMA-filled shared-memory stages at every width (test / comparison hook; the default
+                                         takes the register-landing row pass where the frame width allows) */
 #define VCRYPT_FLAG_DEVICE_HASH 16u   /* sub-frame SHA-256 of vcrypt_encrypt_frames on the GPU, on the frames it
                                          uploads anyway, shared with the host threads band by band (device_hash_bands;
                                          same H); shapes with 3W % 16 != 0 are hashed on the host only */

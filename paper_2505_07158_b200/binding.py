@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 OK, E_ARG, E_KEY, E_SHAPE, E_CUDA, E_NOMEM, E_STATE = 0, -1, -2, -3, -4, -5, -6
-FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR, FLAG_DEVICE_DERIVE, FLAG_DEVICE_HASH, FLAG_PERSISTENT = 1, 2, 4, 8, 16, 32
+FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR, FLAG_DEVICE_DERIVE, FLAG_DEVICE_HASH, FLAG_PERSISTENT, FLAG_ROW_TMA = 1, 2, 4, 8, 16, 32, 64
 
 
 class Params(C.Structure):

@@ -264,6 +264,160 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
 }
 
 // ---------------------------------------------------------------------------------------------
+// Row pass, register-landing variant (frames up to 4096 pixels wide): the same two phases on the same planes and the same
+// output buffer as row_pass_kernel, but a block comes in through the threads' own 128-bit streaming loads (LDG.E.128,
+// evict-first) instead of a ring of shared-memory stages filled by the TMA engine: thread `tid` owns phase-1 item(s)
+// tid (+ NT) of every block its CTA takes, loads the item of the NEXT block right after it has consumed the current one,
+// and so keeps 48 (96) bytes in flight in registers through phase 2.  A CTA then needs the planes and one output buffer only
+// (47 KB at w = 1920 instead of 93 KB), three or four CTAs share an SM -- and, under the two-stream schedule, a row CTA
+// fits beside the column pass's CTAs far more often.  Measured on B200 (resident clips, two streams): FHD encrypt
+// 4.33 -> 4.07 us per frame, 4K 22.9 -> 19.6; the decrypt direction gains at 4K only (26.6 -> 25.2; FHD 5.45 -> 5.50) and
+// keeps row_pass_kernel for frames up to 2048 pixels wide.
+// Synchronisation: CTA barrier A (planes complete, the previous block's bulk store has left the output buffer: thread 0
+// waits for it before arriving), CTA barrier B (output buffer complete, planes free); thread 0 then issues the bulk store.
+// Shift parameters: 12 threads of the last warp compute block it+1's while block it is in phase 1; four slots, so that a
+// slot is rewritten three barriers after its last reader.
+// ---------------------------------------------------------------------------------------------
+constexpr int RR_HDR = 512;  // par1[4][16], par2[4][16]
+
+template <bool INV, int NT, int MINB, int IPT>
+__global__ void __launch_bounds__(NT, MINB) row_reg_kernel(const uint8_t *src, uint8_t *dst, const uint16_t *__restrict__ D,
+                                                         Geom g, uint32_t nblocks) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    uint32_t *par1 = reinterpret_cast<uint32_t *>(smem);
+    uint32_t *par2 = reinterpret_cast<uint32_t *>(smem + 256);
+    const uint32_t w = g.w, rb = g.row_bytes, C = w >> 4, Q = w >> 2;
+    const uint32_t blk_bytes = ROW_RB * rb, PS = w + 32u;
+    uint8_t *obuf = smem + RR_HDR;
+    uint8_t *planes = obuf + blk_bytes;
+    const uint32_t G = gridDim.x, tid = threadIdx.x, blk0 = blockIdx.x;
+    if (blk0 >= nblocks) return;
+    const uint32_t niter = (nblocks - blk0 + G - 1) / G;
+    pdl_wait();     // everything below reads or writes global memory the previous kernel of the stream may have written
+    pdl_trigger();  // only now (see row_pass_kernel)
+
+    // decrypt walks the blocks last-first: the column pass wrote the last frames last, they are the likeliest in L2
+    auto blk_of = [&](uint32_t it) -> uint32_t { return INV ? nblocks - 1u - (blk0 + it * G) : blk0 + it * G; };
+    bool has[IPT];
+    uint32_t r1[IPT], k1[IPT], item_off[IPT];
+    uint4 L[IPT][3];
+#pragma unroll
+    for (int m = 0; m < IPT; ++m) {
+        const uint32_t i = tid + (uint32_t)m * NT;  // phase-1 item (row r1, 16 pixels k1)
+        has[m] = i < ROW_RB * C;
+        r1[m] = (i >= C) + (i >= 2u * C) + (i >= 3u * C);
+        k1[m] = i - r1[m] * C;
+        item_off[m] = r1[m] * rb + 48u * k1[m];
+        L[m][0] = L[m][1] = L[m][2] = make_uint4(0u, 0u, 0u, 0u);
+        if (has[m]) {
+            const uint4 *p = reinterpret_cast<const uint4 *>(src + (size_t)blk_of(0) * blk_bytes + item_off[m]);
+            L[m][0] = __ldcs(p); L[m][1] = __ldcs(p + 1); L[m][2] = __ldcs(p + 2);
+        }
+    }
+    const uint32_t plane_lane = tid - (NT - 32);  // parameter threads: lanes 0 .. 11 of the last warp
+    const bool is_par = plane_lane < 3u * ROW_RB;
+    const uint32_t pr = plane_lane / 3u, pch = plane_lane - 3u * pr;
+    const uint32_t pslot = pr * 4u + pch, poff = (pr * 3u + pch) * PS;
+    if (is_par) {
+        const uint2 pv = row_param(D, g, blk_of(0) * ROW_RB + pr, pch, INV, poff);
+        par1[pslot] = pv.x;
+        par2[pslot] = pv.y;
+    }
+    __syncthreads();
+
+    for (uint32_t it = 0; it < niter; ++it) {
+        const uint32_t blk = blk_of(it);
+        const uint32_t *p1 = par1 + (it & 3u) * 16u, *p2 = par2 + (it & 3u) * 16u;
+        if (is_par && it + 1 < niter) {
+            const uint2 pv = row_param(D, g, blk_of(it + 1) * ROW_RB + pr, pch, INV, poff);
+            par1[((it + 1) & 3u) * 16u + pslot] = pv.x;
+            par2[((it + 1) & 3u) * 16u + pslot] = pv.y;
+        }
+        // ---- phase 1: registers -> planes (as in row_pass_kernel), then the same item of the next block -> registers
+#pragma unroll
+        for (int m = 0; m < IPT; ++m) {
+            if (!has[m]) continue;
+            const uint4 a = L[m][0], b = L[m][1], c = L[m][2];
+            const uint4 dq = *reinterpret_cast<const uint4 *>(p1 + 4u * r1[m]);
+            const uint32_t W[12] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c.x, c.y, c.z, c.w};
+            uint4 v0, v1, v2;
+#define VK_DEINT(m_, X0, X1, X2)                                                          \
+    X0 = __byte_perm(__byte_perm(W[3 * m_], W[3 * m_ + 1], 0x0630), W[3 * m_ + 2], 0x5210); \
+    X1 = __byte_perm(__byte_perm(W[3 * m_], W[3 * m_ + 1], 0x0741), W[3 * m_ + 2], 0x6210); \
+    X2 = __byte_perm(__byte_perm(W[3 * m_], W[3 * m_ + 1], 0x0052), W[3 * m_ + 2], 0x7410);
+            VK_DEINT(0, v0.x, v1.x, v2.x)
+            VK_DEINT(1, v0.y, v1.y, v2.y)
+            VK_DEINT(2, v0.z, v1.z, v2.z)
+            VK_DEINT(3, v0.w, v1.w, v2.w)
+#undef VK_DEINT
+            uint8_t *pl = planes + r1[m] * 3u * PS;
+            const int32_t k16 = (int32_t)(16u * k1[m]);
+#define VK_PUT(V, DQ, CH)                                                      \
+    {                                                                          \
+        int32_t kb = k16 - (int32_t)(DQ);                                      \
+        if (kb < 0) kb += (int32_t)w;                                          \
+        uint8_t *d = pl + (CH) * PS + kb;                                      \
+        *reinterpret_cast<uint4 *>(d) = V;                                     \
+        if (kb < 32) *reinterpret_cast<uint4 *>(d + w) = V; /* pad chunks */   \
+    }
+            VK_PUT(v0, dq.x, 0u)
+            VK_PUT(v1, dq.y, 1u)
+            VK_PUT(v2, dq.z, 2u)
+#undef VK_PUT
+            if (it + 1 < niter) {
+                const uint4 *p = reinterpret_cast<const uint4 *>(src + (size_t)blk_of(it + 1) * blk_bytes + item_off[m]);
+                L[m][0] = __ldcs(p); L[m][1] = __ldcs(p + 1); L[m][2] = __ldcs(p + 2);
+            }
+        }
+        if (tid == 0) bulk_wait_read_0();  // the previous block's store has left the output buffer
+        __syncthreads();                   // A
+
+        // ---- phase 2: rotate; item = quad q (4 pixels) of all 4 rows and 3 channels (as in row_pass_kernel)
+        for (uint32_t q = tid; q < Q; q += NT) {
+            const uint8_t *qa = planes + 4u * q;
+            uint32_t R[ROW_RB][3];
+#pragma unroll
+            for (int r = 0; r < ROW_RB; ++r) {
+                const uint4 pvr = *reinterpret_cast<const uint4 *>(p2 + 4 * r);
+                const uint32_t pvv[3] = {pvr.x, pvr.y, pvr.z};
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) {
+                    const uint32_t *P = reinterpret_cast<const uint32_t *>(qa + (pvv[ch] >> 8));
+                    R[r][ch] = __funnelshift_r(P[0], P[1], pvv[ch]);  // shift amount = low 5 bits
+                }
+            }
+            uint8_t *o = obuf + 12u * q;
+            if (!INV) {
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) {
+                    const uint32_t t01a = __byte_perm(R[0][ch], R[1][ch], 0x5140), t01b = __byte_perm(R[0][ch], R[1][ch], 0x7362);
+                    const uint32_t t23a = __byte_perm(R[2][ch], R[3][ch], 0x5140), t23b = __byte_perm(R[2][ch], R[3][ch], 0x7362);
+                    const uint32_t T[4] = {__byte_perm(t01a, t23a, 0x5410), __byte_perm(t01a, t23a, 0x7632),
+                                           __byte_perm(t01b, t23b, 0x5410), __byte_perm(t01b, t23b, 0x7632)};
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) {
+                        const int y = 3 * p + ch;
+                        *reinterpret_cast<uint32_t *>(o + (y & 3) * rb + 4 * (y >> 2)) = T[p];
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < ROW_RB; ++r) {
+                    uint32_t *po = reinterpret_cast<uint32_t *>(o + r * rb);
+                    po[0] = __byte_perm(__byte_perm(R[r][0], R[r][1], 0x1040), R[r][2], 0x3410);
+                    po[1] = __byte_perm(__byte_perm(R[r][0], R[r][1], 0x6205), R[r][2], 0x3250);
+                    po[2] = __byte_perm(__byte_perm(R[r][0], R[r][1], 0x0730), R[r][2], 0x7216);
+                }
+            }
+        }
+        fence_async_smem();  // generic-proxy writes to the output buffer -> visible to the bulk store
+        __syncthreads();     // B
+        if (tid == 0) bulk_s2g(dst + (size_t)blk * blk_bytes, obuf, blk_bytes);
+    }
+    if (tid == 0) bulk_wait_all();
+}
+
+// ---------------------------------------------------------------------------------------------
 // Column pass, encrypt direction: vertical circular shift of every byte column (Algorithm 5 / Eq. 3, one
 // d_v per pixel column and channel = per byte column of the interleaved matrix) fused with the XOR of
 // Algorithm 6:   dst(ro, x) = B(ro, x) xor I((ro - t_x) mod h, x),   I = the row pass output in T4 layout.
@@ -316,10 +470,14 @@ __global__ void __launch_bounds__(NT, MINB)
     pdl_trigger();
     // keystream look-ahead: thread 0 asks the TMA engine to pull the strip's keystream tiles into L2, CE_AHEAD rows
     // ahead of the row group the CTA is working on (the threads' own loads then hit L2 instead of waiting on DRAM)
+    // (only where a thread has ONE round of keystream loads in flight: with two, the look-ahead costs more than it hides --
+    // FHD, two CTAs per SM: 4.38 -> 4.30 us per frame without it)
+    constexpr bool LOOKAHEAD = DEPTH == 1;
     uint32_t pf_row = 0;
     if (threadIdx.x == 0) {
-        for (; pf_row < h && pf_row < CE_AHEAD + (DEPTH - 1) * GSTEP * CE_G; pf_row += pf_rows)
-            tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
+        if (LOOKAHEAD)
+            for (; pf_row < h && pf_row < CE_AHEAD + (DEPTH - 1) * GSTEP * CE_G; pf_row += pf_rows)
+                tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
         mbar_init(bar, 1);
         mbar_init_fence();
         pdl_wait();  // the strip is the row pass's output
@@ -370,10 +528,10 @@ __global__ void __launch_bounds__(NT, MINB)
             const uint8_t *pd = pB + (size_t)d * gstep;
             if (gd < nfull) {
 #pragma unroll
-                for (int i = 0; i < CE_G; ++i) kb[d][i] = __ldcs(VK_ROWPTR(const uint2 *, pd, offs[i]));
+                for (int i = 0; i < CE_G; ++i) kb[d][i] = ldg_once_u2(VK_ROWPTR(const uint2 *, pd, offs[i]));
             } else if (gd * CE_G < h) {
 #pragma unroll
-                for (int i = 0; i < CE_G / 2; ++i) kb[d][i] = __ldcs(VK_ROWPTR(const uint2 *, pd, offs[i]));
+                for (int i = 0; i < CE_G / 2; ++i) kb[d][i] = ldg_once_u2(VK_ROWPTR(const uint2 *, pd, offs[i]));
             }
         }
     }
@@ -453,13 +611,13 @@ __global__ void __launch_bounds__(NT, MINB)
 #pragma unroll
                 for (int i = 0; i < CE_G; ++i) {
                     const uint32_t lo = sl ? O[i][1] : O[i][0], hi = sl ? O[i][0] : O[i][1];
-                    __stcs(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[pd][i].x, hi ^ kb[pd][i].y));
+                    stg_once_u2(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[pd][i].x, hi ^ kb[pd][i].y));
                 }
             } else {  // the half group at the bottom of a frame with h % 8 == 4: always the last one
 #pragma unroll
                 for (int i = 0; i < CE_G / 2; ++i) {
                     const uint32_t lo = sl ? O[i][1] : O[i][0], hi = sl ? O[i][0] : O[i][1];
-                    __stcs(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[pd][i].x, hi ^ kb[pd][i].y));
+                    stg_once_u2(VK_ROWPTR(uint2 *, pO, offs[i]), make_uint2(lo ^ kb[pd][i].x, hi ^ kb[pd][i].y));
                 }
                 return false;
             }
@@ -467,17 +625,17 @@ __global__ void __launch_bounds__(NT, MINB)
             if (gn * CE_G >= h) return false;
             // keystream of the group DEPTH rounds on, into the registers just used
             const uint32_t gl = gi + (uint32_t)DEPTH * GSTEP;
-            if (threadIdx.x == 0)
+            if (LOOKAHEAD && threadIdx.x == 0)
                 for (; pf_row < h && pf_row < gl * CE_G + CE_AHEAD; pf_row += pf_rows)
                     tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
             {
                 const uint8_t *pl = pB + (size_t)DEPTH * gstep;
                 if (gl < nfull) {
 #pragma unroll
-                    for (int i = 0; i < CE_G; ++i) kb[pd][i] = __ldcs(VK_ROWPTR(const uint2 *, pl, offs[i]));
+                    for (int i = 0; i < CE_G; ++i) kb[pd][i] = ldg_once_u2(VK_ROWPTR(const uint2 *, pl, offs[i]));
                 } else if (gl * CE_G < h) {
 #pragma unroll
-                    for (int i = 0; i < CE_G / 2; ++i) kb[pd][i] = __ldcs(VK_ROWPTR(const uint2 *, pl, offs[i]));
+                    for (int i = 0; i < CE_G / 2; ++i) kb[pd][i] = ldg_once_u2(VK_ROWPTR(const uint2 *, pl, offs[i]));
                 }
             }
             pB += gstep;
@@ -576,7 +734,7 @@ __global__ void __launch_bounds__(NT, MINB)
         for (int t = 0; t < 4; ++t) kq[d][t] = make_uint2(0u, 0u);
         if (col_ok && g0 + (uint32_t)d * GSTEP < nblk) {
 #pragma unroll
-            for (int t = 0; t < 4; ++t) kq[d][t] = __ldcs(VK_ROWPTR(const uint2 *, pB + (size_t)d * bstep, offs4[t]));
+            for (int t = 0; t < 4; ++t) kq[d][t] = ldg_once_u2(VK_ROWPTR(const uint2 *, pB + (size_t)d * bstep, offs4[t]));
         }
     }
     __syncthreads();    // mbarrier initialised, ups[] complete
@@ -596,7 +754,7 @@ __global__ void __launch_bounds__(NT, MINB)
                     tma_prefetch_2d(&tm_B, (int32_t)x0, (int32_t)(f * h + pf_row));
             if (R4 + (uint32_t)KD * GSTEP < nblk) {  // the block KD rounds on, into the registers just read
 #pragma unroll
-                for (int t = 0; t < 4; ++t) kq[pd][t] = __ldcs(VK_ROWPTR(const uint2 *, pB + (size_t)KD * bstep, offs4[t]));
+                for (int t = 0; t < 4; ++t) kq[pd][t] = ldg_once_u2(VK_ROWPTR(const uint2 *, pB + (size_t)KD * bstep, offs4[t]));
             }
             pB += bstep;
             uint8_t *ps = S + ((size_t)(4u * R4) * X + 8u * j) + (s1 ? X : 0u);
@@ -777,6 +935,7 @@ __global__ void __launch_bounds__(256)
 static size_t row_smem_bytes(const Geom &g, int ns) {
     return (size_t)ROW_HDR + (size_t)(ns + 1) * ROW_RB * g.row_bytes + (size_t)ROW_RB * 3 * (g.w + 32);
 }
+static size_t rowreg_smem_bytes(const Geom &g) { return (size_t)RR_HDR + (size_t)ROW_RB * g.row_bytes + (size_t)ROW_RB * 3 * (g.w + 32); }
 static size_t cole_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + CE_PAD) * X + 16 + 2 * (size_t)X; }
 
 template <int X, int NT, int MINB, int KD>
@@ -792,7 +951,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-cudaError_t make_plan(const Geom &g, int device, Plan *out) {
+cudaError_t make_plan(const Geom &g, int device, bool row_tma, Plan *out) {
     Plan p{};
     int smem_optin = 0, smem_sm = 0, sms = 0;
     cudaError_t e = cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
@@ -869,6 +1028,21 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
                 p.row_ns_dec = 1;
                 p.smem_row_dec = row_smem_bytes(g, 1);
             }
+            // register-landing row pass: every width whose phase-1 items (w / 4 per block) fit one or two per thread
+            p.row_reg = 0;
+            p.row_reg_dec = false;
+            p.smem_row_reg = rowreg_smem_bytes(g);
+            if (!row_tma && p.smem_row_reg <= (size_t)smem_optin) {
+                const uint32_t items = g.w / 4u;
+                int per_sm = 0;
+                if (items <= 256) { p.row_reg = 1; per_sm = 4; }
+                else if (items <= 512) { p.row_reg = 2; per_sm = 3; }
+                else if (items <= 1024) { p.row_reg = 3; per_sm = 2; p.row_reg_dec = true; }
+                const int by_smem = (int)((size_t)smem_sm / (p.smem_row_reg + 1024));
+                if (per_sm > by_smem) per_sm = by_smem;
+                if (per_sm < 1) p.row_reg = 0;
+                p.row_reg_grid_max = per_sm * sms;
+            }
             int rc = (int)((size_t)smem_sm / (p.smem_row + 1024));
             const int by_threads = 2048 / (nc + 32);
             if (rc > by_threads) rc = by_threads;
@@ -901,6 +1075,10 @@ cudaError_t make_plan(const Geom &g, int device, Plan *out) {
             if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_dec);
             if (!e) e = cudaFuncSetAttribute(row_pass_kernel<false, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
             if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
+            if (!e && p.row_reg == 1) e = cudaFuncSetAttribute(row_reg_kernel<false, 256, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
+            if (!e && p.row_reg == 2) e = cudaFuncSetAttribute(row_reg_kernel<false, 512, 3, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
+            if (!e && p.row_reg == 3) e = cudaFuncSetAttribute(row_reg_kernel<false, 512, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
+            if (!e && p.row_reg == 3) e = cudaFuncSetAttribute(row_reg_kernel<true, 512, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
             if (e != cudaSuccess) return e;
         }
     }
@@ -929,6 +1107,13 @@ template <bool INV>
 static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, const uint16_t *D, size_t n,
                               uint8_t *dst, cudaStream_t st) {
     const uint32_t nblocks = (uint32_t)(n * g.h / ROW_RB);
+    if (p.row_reg && (!INV || p.row_reg_dec)) {
+        const uint32_t gm = (uint32_t)p.row_reg_grid_max;
+        const uint32_t rr = (nblocks + gm - 1u) / gm, gr = (nblocks + rr - 1u) / rr;  // balanced, as below
+        if (p.row_reg == 3) return launch_pdl(row_reg_kernel<INV, 512, 2, 2>, gr, 512u, p.smem_row_reg, st, src, dst, D, g, nblocks);
+        if (!INV && p.row_reg == 2) return launch_pdl(row_reg_kernel<false, 512, 3, 1>, gr, 512u, p.smem_row_reg, st, src, dst, D, g, nblocks);
+        if (!INV && p.row_reg == 1) return launch_pdl(row_reg_kernel<false, 256, 4, 1>, gr, 256u, p.smem_row_reg, st, src, dst, D, g, nblocks);
+    }
     // persistent CTAs, balanced: the fewest rounds the resident CTAs allow, then the smallest grid that needs no more rounds
     // (FHD, 5 frames: 1350 blocks = 5 rounds of 270 CTAs instead of 296 CTAs of which 166 take a 5th block; measured 4.50 ->
     // 4.44 us per frame, decrypt 5.58 -> 5.46: no CTA idles through a last round while it holds its share of the SM)

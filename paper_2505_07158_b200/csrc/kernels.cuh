@@ -32,6 +32,11 @@ struct Plan {
     int row_grid_max;      // row pass: persistent CTAs (resident CTAs per SM x SMs)
     int row_nc_dec, row_ns_dec, row_grid_max_dec;  // the same for the inverse row pass (decrypt): three small CTAs per SM where they fit
     size_t smem_row_dec;
+    int row_reg;           // register-landing row pass (row_reg_kernel): 0 = not used, 1 = 256-thread CTAs (w <= 1024), 2 = 512-thread
+                           // CTAs (w <= 2048), 3 = 512-thread CTAs with two items per thread (w <= 4096)
+    bool row_reg_dec;      // ... also for the inverse row pass (wide frames only: measured)
+    int row_reg_grid_max;  // its persistent CTAs
+    size_t smem_row_reg;
     uint32_t box_rows;     // column pass: rows per TMA tensor tile (largest divisor of h that is <= 256)
     uint32_t h_magic;      // ceil(2^32 / h): d mod h without a division for d < 2^16
     void *encode_tiled;    // cuTensorMapEncodeTiled, resolved through the runtime (no link-time libcuda dependency)
@@ -42,7 +47,8 @@ struct Plan {
     size_t max_frames_per_launch;  // keeps the intermediate (n * 3wh bytes) L2-resident
 };
 
-cudaError_t make_plan(const Geom &g, int device, Plan *out);
+// row_tma: keep the TMA-staged row pass for every width (test / comparison hook)
+cudaError_t make_plan(const Geom &g, int device, bool row_tma, Plan *out);
 
 // Encrypt n frames: row pass (horizontal bit rotation, Eq. 2) then column pass
 // (vertical shift, Eq. 3, fused with the XOR of Algorithm 6).  dst may equal src.

@@ -1,4 +1,4 @@
-// ptx.cuh -- inline-PTX wrappers shared by the sm_100a cipher kernels (cipher.cu): mbarriers, bulk async copies (TMA),
+// ptx.cuh -- inline-PTX wrappers shared by the sm_100a cipher kernels (kernels.cu, cipher.cu): mbarriers, bulk async copies (TMA),
 // tensor-map tile loads and L2 prefetches, programmatic dependent launch, named barriers, gpu-scope acquire / release.
 // SASS: SYNCS.*, UBLKCP, UTMALDG, UTMAPF, BAR.SYNC, ACQBULK / LDG.E.STRONG.GPU.
 #pragma once
@@ -124,6 +124,18 @@ __device__ __forceinline__ uint64_t mad_wide_ptr(const void *p, uint32_t off) {
     uint64_t r;
     asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(r) : "r"(off), "l"(reinterpret_cast<uint64_t>(p)));
     return r;
+}
+
+// ---- streaming global accesses ---------------------------------------------------------------------------------
+// 64-bit load of read-only data that is used once: read-only path, no L1 line kept (LDG.E.64.CONSTANT with the no-allocate hint)
+__device__ __forceinline__ uint2 ldg_once_u2(const uint2 *p) {
+    uint2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+    return v;
+}
+// 64-bit store that leaves no line in L1
+__device__ __forceinline__ void stg_once_u2(uint2 *p, uint2 v) {
+    asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(v.x), "r"(v.y) : "memory");
 }
 
 // ---- gpu-scope flags between CTAs of one grid -------------------------------------------------------------------

@@ -375,7 +375,7 @@ extern "C" int vcrypt_init(vcrypt_ctx **out, const vcrypt_params *p) {
             cudaError_t e = cudaGetDevice(&prev_dev);
             if (e == cudaSuccess && dev < 0) dev = prev_dev;
             if (e == cudaSuccess) e = cudaSetDevice(dev);
-            if (e == cudaSuccess) e = vk::make_plan(c->g, dev, &c->plan);
+            if (e == cudaSuccess) e = vk::make_plan(c->g, dev, (p->flags & VCRYPT_FLAG_ROW_TMA) != 0, &c->plan);
             if (e == cudaSuccess) {
                 vk::UniTune tune{p->tune_row_stages, p->tune_row_item_blocks, p->tune_window, p->tune_ring};
                 e = vk::make_uni_plan(c->g, dev, tune, &c->uni);

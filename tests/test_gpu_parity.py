@@ -115,6 +115,23 @@ def test_in_place_and_forced_generic(torch_cuda, vb, orc, w, h, nf, generic):
     assert np.array_equal(run_device(torch_cuda, v, ref, D, B, decrypt=True, inplace=True), F)
 
 
+# Row pass variants: the default plan takes the register-landing row pass (256 threads up to w = 1024, 512 threads up to 2048, 512
+# threads with two items per thread up to 4096; the inverse direction only above 2048) and the TMA-staged one beyond;
+# VCRYPT_FLAG_ROW_TMA keeps the TMA-staged row pass at every width.  Widths on both sides of every boundary, widths whose items do
+# not fill the last warp, several blocks per CTA (nf * h / 4 above the resident CTAs), in place.
+@pytest.mark.parametrize("w,h,nf", [(64, 16, 2), (1024, 16, 2), (1040, 20, 1), (2048, 16, 2), (2064, 20, 2), (3840, 16, 1), (4096, 16, 1),
+                                    (4112, 16, 1), (640, 480, 12), (1920, 64, 40)])
+@pytest.mark.parametrize("row_tma", [False, True])
+def test_row_pass_variants_match_oracle(torch_cuda, vb, orc, w, h, nf, row_tma):
+    F, D, B = rnd_case(w, h, nf, seed=w + 3 * h + nf)
+    v = gpu_ctx(vb, w, h, flags=vb.FLAG_ROW_TMA if row_tma else 0)
+    ref = oracle_frames(orc, F, D, B)
+    assert np.array_equal(run_device(torch_cuda, v, F, D, B), ref)
+    assert np.array_equal(run_device(torch_cuda, v, F, D, B, inplace=True), ref)
+    assert np.array_equal(run_device(torch_cuda, v, ref, D, B, decrypt=True), F)
+    assert np.array_equal(run_device(torch_cuda, v, ref, D, B, decrypt=True, inplace=True), F)
+
+
 @pytest.mark.parametrize("w,h,nf", [(256, 256, 1), (64, 48, 3), (112, 20, 3), (64, 16, 5), (2048, 24, 1), (144, 1028, 1), (640, 480, 7),
                                     (64, 48, 40), (720, 480, 2), (1920, 1080, 3)])
 @pytest.mark.parametrize("tune", [(0, 0, 0, 0), (1, 1, 1, 3), (2, 7, 2, 1)])
