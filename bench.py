@@ -69,10 +69,10 @@ class ClockSampler:
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int):
+    def __init__(self, index: int, period_ms: int = 100):
         self.p = None
         try:
-            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", str(period_ms),
                                        "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
             self.p = None
@@ -152,7 +152,7 @@ def workload_name(cfg):
             f"key = 4 doubles, n_workers = {synth.N_WORKERS}")
 
 
-def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, hold_ms=50.0):
+def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, sustained_ms=1000.0, idle_s=0.5):
     """Kernel-only timing on a resident clip: encrypt as ONE call (the library's resident-clip schedule), encrypt as one call
     per batch of cfg.batch frames on one stream (config 4 as BASELINE.json words it), decrypt as one call.  CUDA events on
     the calling stream.  Returns a dict; the ciphertext is left in d_E."""
@@ -176,14 +176,15 @@ def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, hold_ms=5
             n += kctx.launch_count()[0]
         return n
 
-    # W untimed steps, held for at least hold_ms of GPU work: the timed steps must not see the clock ramp of a GPU that idled
-    # during the host-side set-up (a kernel-only step lasts about a millisecond)
-    warm_steps, t_warm = 0, _t.perf_counter()
-    while warm_steps < W or (_t.perf_counter() - t_warm < hold_ms * 1e-3 and warm_steps < 2000):
+    # W untimed steps, then the K timed ones: a burst of a few milliseconds on a GPU that idled through the host-side set-up,
+    # which is how MEASURED_PEAKS.json's copy rate was taken (best of 10 copies).  Under continuous load the power cap lowers
+    # the SM clock within 50 - 150 ms (1965 -> about 1600 MHz) and this path, which is bound by latencies and issue slots more than
+    # by DRAM, slows down more than a plain copy does: the `sustained` leg below measures both after `sustained_ms` of load.
+    warm_steps = 0
+    while warm_steps < W:
         clip_step()
         warm_steps += 1
-        if warm_steps >= W:
-            torch.cuda.synchronize()
+    torch.cuda.synchronize()
     barrier()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
     launches = 0
@@ -201,6 +202,8 @@ def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, hold_ms=5
 
     KB = max(1, min(K, 5))
     d_E.zero_()
+    torch.cuda.synchronize()
+    _t.sleep(idle_s)  # every leg starts from an idle GPU: its number must not depend on the legs before it
     for _ in range(2):
         batch_step()
     barrier()
@@ -217,6 +220,8 @@ def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, hold_ms=5
     out["batches_same"] = bool(synth.digest(d_E.cpu().numpy()) == out["digest_all"])
 
     d_P = torch.empty_like(d_F)
+    torch.cuda.synchronize()
+    _t.sleep(idle_s)
     for _ in range(2):
         kctx.decrypt_device(d_E, d_D, d_B, d_P, stream)
     barrier()
@@ -229,6 +234,30 @@ def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, hold_ms=5
     out["dec_ms_frame"] = dv[0].elapsed_time(dv[1]) / KB / T
     out["dec_steps"] = KB
     out["decrypt_ok"] = bool(torch.equal(d_P, d_F))
+
+    # sustained: the same clip step after `sustained_ms` of continuous load, and a plain device copy of the clip under the same
+    # conditions (torch's copy kernel, what MEASURED_PEAKS.json times) -- context for the burst figures above
+    if sustained_ms > 0:
+        def held(step):
+            torch.cuda.synchronize()
+            _t.sleep(idle_s)
+            t0 = _t.perf_counter()
+            while _t.perf_counter() - t0 < sustained_ms * 1e-3:
+                step()
+                torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(K):
+                step()
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / K
+        out["sustained_step_ms"] = held(clip_step)
+        out["sustained_copy_ms"] = held(lambda: d_P.copy_(d_F))
+        out["sustained_copy_gbs"] = 2.0 * d_F.numel() / (out["sustained_copy_ms"] * 1e-3) / 1e9
+        out["sustained_hold_ms"] = sustained_ms
+        torch.cuda.synchronize()
+        _t.sleep(idle_s)
     out["d_E"] = d_E
     kctx.destroy()
     return out
@@ -248,6 +277,8 @@ def c5_leg(vb, torch, peak, frames=40, steps=3):
     alg = 9 * cfg.w * cfg.h + 6 * (cfg.w + cfg.h)
     res = {"workload": f"C5 shape {cfg.w}x{cfg.h}x3, resident clip of {frames} frames, one call per direction, random D and B", "steps": steps}
     for name, fn, src, dst in (("encrypt", v.encrypt_device, F, E), ("decrypt", v.decrypt_device, E, P)):
+        torch.cuda.synchronize()
+        time.sleep(0.5)  # from an idle GPU, like the other kernel-only legs
         for _ in range(3):
             fn(src, D, B, dst)
         torch.cuda.synchronize()
@@ -342,6 +373,7 @@ def main():
     ap.add_argument("--no-extra-legs", action="store_true", help="skip the bounded C5 (4K) and C3 (single-frame latency) legs")
     ap.add_argument("--kernel-leg-only", action="store_true",
                     help="only the kernel-only legs, exactly --warmup untimed steps: the command profiles/ captures under ncu")
+    ap.add_argument("--clock-sample-ms", type=int, default=100, help="period of the nvidia-smi clock / throttle-reason samples")
     ap.add_argument("--persistent", action="store_true", help="kernel-only legs through the persistent kernel (VCRYPT_FLAG_PERSISTENT)")
     ap.add_argument("--derive", default="auto", choices=["auto", "host", "device"],
                     help="where the worker systems (D, B) of the end-to-end leg run: host lanes or the GPU (same bytes)")
@@ -414,8 +446,8 @@ def main():
     del B_all
 
     # ---- kernel-only legs: CUDA events on the launching stream ---------------------------------------------
-    sampler = ClockSampler(local) if rank == 0 else None
-    kl = kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, hold_ms=0.0 if args.kernel_leg_only else 50.0)
+    sampler = ClockSampler(local, args.clock_sample_ms) if rank == 0 else None
+    kl = kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, sustained_ms=0.0 if args.kernel_leg_only else 1000.0)
     kern_ms_total = kl["total_ms"]
     pairs_per_step = max(1, kl["launches"] // (2 * K)) if not args.persistent else max(1, kl["launches"] // K)
     if args.kernel_leg_only:
@@ -553,7 +585,7 @@ def main():
     batches_frac = alg_bytes_frame / (kl["batches_ms_frame"] * 1e-3) / 1e9 / peak
     dec_frac = alg_bytes_frame / (kl["dec_ms_frame"] * 1e-3) / 1e9 / peak
     kernel_name = ("cipher_kernel (persistent: row team + strip team per SM)" if args.persistent else
-                   "row_pass_kernel<false> + col_enc_kernel<64> = one launch pair of vcrypt_encrypt_device (col_enc_kernel is the larger "
+                   "row_reg_kernel<false> + col_enc_kernel<64> = one launch pair of vcrypt_encrypt_device (col_enc_kernel is the larger "
                    f"share{'' if col_share is None else f', {col_share:.0%} of a pair in profiles/'})")
     pcie_fps = world * T / pcie_s if pcie_s else None
     out = {
@@ -600,7 +632,15 @@ def main():
                                                "us_per_call": 1e3 * kl["batches_ms_frame"] * min(cfg.batch, T),
                                                "frac": batches_frac, "steps": kl["batches_steps"]},
                      "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
-                     "step_ms_median": statistics.median(kl["step_ms"]), "step_ms_min": min(kl["step_ms"])},
+                     "step_ms_median": statistics.median(kl["step_ms"]), "step_ms_min": min(kl["step_ms"]),
+                     "timed_region": f"{W} warm-up steps, then {K} steps back to back on a GPU that idled before: a burst, like the copies "
+                                     "MEASURED_PEAKS.json's peak is the best of; `sustained` = the same step after a second of continuous load "
+                                     "(the power cap lowers the SM clock), beside a plain device copy of the clip under the same load",
+                     "sustained": None if "sustained_step_ms" not in kl else {
+                         "hold_ms": kl["sustained_hold_ms"], "us_per_frame": 1e3 * kl["sustained_step_ms"] / T,
+                         "frac_of_peak": alg_bytes_frame * T / (kl["sustained_step_ms"] * 1e-3) / 1e9 / peak,
+                         "copy_gbs_same_load": kl["sustained_copy_gbs"],
+                         "frac_of_copy_same_load": alg_bytes_frame * T / (kl["sustained_step_ms"] * 1e-3) / 1e9 / kl["sustained_copy_gbs"]}},
         "e2e_decrypt": {"value": world * T / min(dec_s), "unit": UNIT, "ms_per_frame": 1e3 * min(dec_s) / T,
                         "note": "vcrypt_decrypt_frames from the start of the chain, best of 3 after one warm-up call, pinned host in/out, rank 0's time"},
         "decrypt_kernels": {"value": 1e3 / kl["dec_ms_frame"], "unit": UNIT, "us_per_frame": 1e3 * kl["dec_ms_frame"],

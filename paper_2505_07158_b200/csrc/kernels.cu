@@ -76,13 +76,19 @@ constexpr int ROW_MAXNS = 4;    // stages at most
 // words q + fine, q + fine + 1 of the pre-rotated plane (never wrapping: two pad chunks repeat chunks 0 and 1).
 //   p1 = 16 * dq                      (bytes; phase 1)
 //   p2 = (plane offset + 4 * fine) << 8 | sh5   (phase 2: one LEA.HI gives the address, the funnel shift takes sh5)
-__device__ __forceinline__ uint2 row_param(const uint16_t *__restrict__ D, const Geom &g, uint32_t grow, uint32_t ch,
-                                           bool inv, uint32_t plane_off) {
-    const uint32_t f = grow / g.h, i = grow - f * g.h, W8 = 8u * g.w;
-    const uint32_t s = (uint32_t)D[(size_t)f * g.nD + ch * (g.h + g.w) + i] % W8;
+__device__ __forceinline__ uint32_t row_dist(const uint16_t *__restrict__ D, const Geom &g, uint32_t grow, uint32_t ch) {
+    const uint32_t f = grow / g.h, i = grow - f * g.h;
+    return (uint32_t)D[(size_t)f * g.nD + ch * (g.h + g.w) + i];  // d_h of (frame f, row i, channel ch)
+}
+__device__ __forceinline__ uint2 row_param_of(uint32_t d, const Geom &g, bool inv, uint32_t plane_off) {
+    const uint32_t W8 = 8u * g.w, s = d % W8;
     const uint32_t sh = inv ? s : (s ? W8 - s : 0u);
     const uint32_t dw = sh >> 5;
     return make_uint2((dw >> 2) << 4, ((plane_off + 4u * (dw & 3u)) << 8) | (sh & 31u));
+}
+__device__ __forceinline__ uint2 row_param(const uint16_t *__restrict__ D, const Geom &g, uint32_t grow, uint32_t ch,
+                                           bool inv, uint32_t plane_off) {
+    return row_param_of(row_dist(D, g, grow, ch), g, inv, plane_off);
 }
 
 template <bool INV, int MAXT, int MINB>
@@ -318,20 +324,23 @@ __global__ void __launch_bounds__(NT, MINB) row_reg_kernel(const uint8_t *src, u
     const bool is_par = plane_lane < 3u * ROW_RB;
     const uint32_t pr = plane_lane / 3u, pch = plane_lane - 3u * pr;
     const uint32_t pslot = pr * 4u + pch, poff = (pr * 3u + pch) * PS;
+    uint32_t dnext = 0;  // parameter threads: the distance of block it + 1, loaded one iteration before it is turned into parameters
     if (is_par) {
         const uint2 pv = row_param(D, g, blk_of(0) * ROW_RB + pr, pch, INV, poff);
         par1[pslot] = pv.x;
         par2[pslot] = pv.y;
+        if (niter > 1) dnext = row_dist(D, g, blk_of(1) * ROW_RB + pr, pch);
     }
     __syncthreads();
 
     for (uint32_t it = 0; it < niter; ++it) {
         const uint32_t blk = blk_of(it);
         const uint32_t *p1 = par1 + (it & 3u) * 16u, *p2 = par2 + (it & 3u) * 16u;
-        if (is_par && it + 1 < niter) {
-            const uint2 pv = row_param(D, g, blk_of(it + 1) * ROW_RB + pr, pch, INV, poff);
+        if (is_par && it + 1 < niter) {  // no global-memory latency between the parameter threads and barrier A
+            const uint2 pv = row_param_of(dnext, g, INV, poff);
             par1[((it + 1) & 3u) * 16u + pslot] = pv.x;
             par2[((it + 1) & 3u) * 16u + pslot] = pv.y;
+            if (it + 2 < niter) dnext = row_dist(D, g, blk_of(it + 2) * ROW_RB + pr, pch);
         }
         // ---- phase 1: registers -> planes (as in row_pass_kernel), then the same item of the next block -> registers
 #pragma unroll
@@ -444,6 +453,9 @@ __global__ void __launch_bounds__(NT, MINB) row_reg_kernel(const uint8_t *src, u
 #endif
 #ifndef VK_DE1
 #define VK_DE1 2
+#endif
+#ifndef VK_DE2
+#define VK_DE2 2
 #endif
 constexpr int CE_PAD = 8;   // repeated strip rows
 constexpr int CE_G = 8;     // output rows per group
@@ -646,7 +658,8 @@ __global__ void __launch_bounds__(NT, MINB)
     };
     for (;;) {
         if (!round(std::integral_constant<int, 0>{})) break;
-        if (DEPTH > 1 && !round(std::integral_constant<int, DEPTH - 1>{})) break;
+        if (DEPTH > 1 && !round(std::integral_constant<int, (DEPTH > 1 ? 1 : 0)>{})) break;
+        if (DEPTH > 2 && !round(std::integral_constant<int, (DEPTH > 2 ? 2 : 0)>{})) break;
     }
 #undef VK_ROWPTR
 }
@@ -1063,7 +1076,7 @@ cudaError_t make_plan(const Geom &g, int device, bool row_tma, Plan *out) {
             const size_t l2_budget = (size_t)100 << 20;
             p.max_frames_per_launch = l2_budget / g.frame_bytes ? l2_budget / g.frame_bytes : 1;
             if (ctas == 3) {
-                if (X == 64) { e = col_set_attr<64, 256, 3, VK_KD3>(p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3, 1>(p.smem_cole_enc); if (!e) e = cole_set_attr<64, 256, 2, 2>(p.smem_cole_enc); }
+                if (X == 64) { e = col_set_attr<64, 256, 3, VK_KD3>(p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3, 1>(p.smem_cole_enc); if (!e) e = cole_set_attr<64, 256, 2, VK_DE2>(p.smem_cole_enc); }
                 else { e = col_set_attr<32, 256, 3, VK_KD3>(p.smem_cole); if (!e) e = cole_set_attr<32, 256, 3, 1>(p.smem_cole_enc); }
             } else {
                 if (X == 64) { e = col_set_attr<64, 512, 1, VK_KD1>(p.smem_cole); if (!e) e = cole_set_attr<64, 512, 1, VK_DE1>(p.smem_cole_enc); }
@@ -1189,7 +1202,7 @@ static cudaError_t launch_col_enc(const Geom &g, const Plan &p, uint8_t *io, con
                       (uint32_t)p.strips_per_frame, (uint32_t)n, p.box_rows, p.h_magic, pbox)
     if (p.col_ctas_per_sm == 3) {
         // two CTAs per SM (the larger shared-memory request): registers for two rounds of keystream in flight per thread
-        if (p.strip_bytes == 64 && p.smem_cole_enc != p.smem_cole) VK_COLE(64, 256, 2, 2);
+        if (p.strip_bytes == 64 && p.smem_cole_enc != p.smem_cole) VK_COLE(64, 256, 2, VK_DE2);
         else if (p.strip_bytes == 64) VK_COLE(64, 256, 3, 1);
         else VK_COLE(32, 256, 3, 1);
     } else {
