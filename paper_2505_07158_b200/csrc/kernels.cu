@@ -277,8 +277,8 @@ __global__ void __launch_bounds__(MAXT, MINB) row_pass_kernel(const uint8_t *src
 // and so keeps 48 (96) bytes in flight in registers through phase 2.  A CTA then needs the planes and one output buffer only
 // (47 KB at w = 1920 instead of 93 KB), three or four CTAs share an SM -- and, under the two-stream schedule, a row CTA
 // fits beside the column pass's CTAs far more often.  Measured on B200 (resident clips, two streams): FHD encrypt
-// 4.33 -> 4.07 us per frame, 4K 22.9 -> 19.6; the decrypt direction gains at 4K only (26.6 -> 25.2; FHD 5.45 -> 5.50) and
-// keeps row_pass_kernel for frames up to 2048 pixels wide.
+// 4.33 -> 4.07 us per frame, 4K 22.9 -> 19.6; the decrypt direction takes it too, except for frames 1537 to 2048
+// pixels wide, where row_pass_kernel as three small CTAs per SM is as fast or faster (make_plan).
 // Synchronisation: CTA barrier A (planes complete, the previous block's bulk store has left the output buffer: thread 0
 // waits for it before arriving), CTA barrier B (output buffer complete, planes free); thread 0 then issues the bulk store.
 // Shift parameters: 12 threads of the last warp compute block it+1's while block it is in phase 1; four slots, so that a
@@ -446,7 +446,7 @@ __global__ void __launch_bounds__(NT, MINB) row_reg_kernel(const uint8_t *src, u
 // keystream prefetch depths (rounds of loads in flight per thread): decrypt column pass with three CTAs per SM / one CTA per
 // SM, encrypt column pass with one CTA per SM (development builds may override)
 #ifndef VK_KD3
-#define VK_KD3 2
+#define VK_KD3 3
 #endif
 #ifndef VK_KD1
 #define VK_KD1 3
@@ -1050,11 +1050,16 @@ cudaError_t make_plan(const Geom &g, int device, bool row_tma, Plan *out) {
                 int per_sm = 0;
                 if (items <= 256) { p.row_reg = 1; per_sm = 4; }
                 else if (items <= 512) { p.row_reg = 2; per_sm = 3; }
-                else if (items <= 1024) { p.row_reg = 3; per_sm = 2; p.row_reg_dec = true; }
+                else if (items <= 1024) { p.row_reg = 3; per_sm = 2; }
                 const int by_smem = (int)((size_t)smem_sm / (p.smem_row_reg + 1024));
                 if (per_sm > by_smem) per_sm = by_smem;
                 if (per_sm < 1) p.row_reg = 0;
                 p.row_reg_grid_max = per_sm * sms;
+                // inverse direction: everywhere except frames 1537 to 2048 pixels wide, where the TMA-staged pass as three small CTAs per
+                // SM (row_ns_dec == 1) is as fast or faster.  Measured decrypt, TMA-staged -> register-landing, us per frame on resident
+                // clips: 640 x 480 0.84 -> 0.75, 1024 x 768 1.99 -> 1.90, 1280 x 720 2.27 -> 2.21, 3840 x 2160 26.6 -> 25.2, but
+                // 1760 x 992 4.30 -> 4.33, 1920 x 1080 4.95 -> 5.07, 2048 x 1080 5.40 -> 5.46.
+                p.row_reg_dec = p.row_reg != 0 && !(p.row_ns_dec == 1 && g.w > 1536);
             }
             int rc = (int)((size_t)smem_sm / (p.smem_row + 1024));
             const int by_threads = 2048 / (nc + 32);
@@ -1089,7 +1094,9 @@ cudaError_t make_plan(const Geom &g, int device, bool row_tma, Plan *out) {
             if (!e) e = cudaFuncSetAttribute(row_pass_kernel<false, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
             if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
             if (!e && p.row_reg == 1) e = cudaFuncSetAttribute(row_reg_kernel<false, 256, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
+            if (!e && p.row_reg == 1) e = cudaFuncSetAttribute(row_reg_kernel<true, 256, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
             if (!e && p.row_reg == 2) e = cudaFuncSetAttribute(row_reg_kernel<false, 512, 3, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
+            if (!e && p.row_reg == 2) e = cudaFuncSetAttribute(row_reg_kernel<true, 512, 3, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
             if (!e && p.row_reg == 3) e = cudaFuncSetAttribute(row_reg_kernel<false, 512, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
             if (!e && p.row_reg == 3) e = cudaFuncSetAttribute(row_reg_kernel<true, 512, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
             if (e != cudaSuccess) return e;
@@ -1124,8 +1131,8 @@ static cudaError_t launch_row(const Geom &g, const Plan &p, const uint8_t *src, 
         const uint32_t gm = (uint32_t)p.row_reg_grid_max;
         const uint32_t rr = (nblocks + gm - 1u) / gm, gr = (nblocks + rr - 1u) / rr;  // balanced, as below
         if (p.row_reg == 3) return launch_pdl(row_reg_kernel<INV, 512, 2, 2>, gr, 512u, p.smem_row_reg, st, src, dst, D, g, nblocks);
-        if (!INV && p.row_reg == 2) return launch_pdl(row_reg_kernel<false, 512, 3, 1>, gr, 512u, p.smem_row_reg, st, src, dst, D, g, nblocks);
-        if (!INV && p.row_reg == 1) return launch_pdl(row_reg_kernel<false, 256, 4, 1>, gr, 256u, p.smem_row_reg, st, src, dst, D, g, nblocks);
+        if (p.row_reg == 2) return launch_pdl(row_reg_kernel<INV, 512, 3, 1>, gr, 512u, p.smem_row_reg, st, src, dst, D, g, nblocks);
+        if (p.row_reg == 1) return launch_pdl(row_reg_kernel<INV, 256, 4, 1>, gr, 256u, p.smem_row_reg, st, src, dst, D, g, nblocks);
     }
     // persistent CTAs, balanced: the fewest rounds the resident CTAs allow, then the smallest grid that needs no more rounds
     // (FHD, 5 frames: 1350 blocks = 5 rounds of 270 CTAs instead of 296 CTAs of which 166 take a 5th block; measured 4.50 ->

@@ -116,10 +116,11 @@ def test_in_place_and_forced_generic(torch_cuda, vb, orc, w, h, nf, generic):
 
 
 # Row pass variants: the default plan takes the register-landing row pass (256 threads up to w = 1024, 512 threads up to 2048, 512
-# threads with two items per thread up to 4096; the inverse direction only above 2048) and the TMA-staged one beyond;
+# threads with two items per thread up to 4096; the inverse direction too, except for frames 1537 to 2048 pixels wide) and the
+# TMA-staged one beyond;
 # VCRYPT_FLAG_ROW_TMA keeps the TMA-staged row pass at every width.  Widths on both sides of every boundary, widths whose items do
 # not fill the last warp, several blocks per CTA (nf * h / 4 above the resident CTAs), in place.
-@pytest.mark.parametrize("w,h,nf", [(64, 16, 2), (1024, 16, 2), (1040, 20, 1), (2048, 16, 2), (2064, 20, 2), (3840, 16, 1), (4096, 16, 1),
+@pytest.mark.parametrize("w,h,nf", [(64, 16, 2), (1024, 16, 2), (1040, 20, 1), (1536, 16, 2), (1552, 16, 2), (2048, 16, 2), (2064, 20, 2), (3840, 16, 1), (4096, 16, 1),
                                     (4112, 16, 1), (640, 480, 12), (1920, 64, 40)])
 @pytest.mark.parametrize("row_tma", [False, True])
 def test_row_pass_variants_match_oracle(torch_cuda, vb, orc, w, h, nf, row_tma):
@@ -302,6 +303,33 @@ def test_resident_clip_schedule_defaults(torch_cuda, vb, orc):
     assert np.array_equal(run_device(torch_cuda, v, E, D, B, decrypt=True), F)
     E2 = run_device(torch_cuda, v, F[:120], D[:120], B[:120])
     assert v.launch_count()[0] == 4 and np.array_equal(E2, E[:120])
+
+
+@pytest.mark.parametrize("w,h,nf", [(640, 480, 6), (1920, 1080, 3), (64, 48, 9), (100, 37, 3)])
+def test_calls_chained_on_one_stream_without_host_sync(torch_cuda, vb, orc, w, h, nf):
+    """Every kernel of the library starts under programmatic dependent launch: a call's first kernel may be scheduled while the
+    last kernel of the call before it (which lets its dependents launch early) is still running.  Producer -> consumer chains on one
+    stream with no host synchronisation in between: the inputs D and B written by device copies right before the call, encrypt ->
+    decrypt -> encrypt in place on the same buffers, repeated; the result must be what the oracle gives for the last inputs."""
+    torch = torch_cuda
+    F, D, B = rnd_case(w, h, nf, seed=77)
+    F2, D2, B2 = rnd_case(w, h, nf, seed=78)
+    v = gpu_ctx(vb, w, h)
+    src = [torch.from_numpy(a).cuda() for a in (F, D.view(np.int16), B)]
+    src2 = [torch.from_numpy(a).cuda() for a in (F2, D2.view(np.int16), B2)]
+    dF, dD, dB = (torch.empty_like(t) for t in src)
+    dE, dP = torch.empty_like(dF), torch.empty_like(dF)
+    torch.cuda.synchronize()
+    for rep in range(6):
+        cur = src if rep % 2 == 0 else src2
+        dF.copy_(cur[0]); dD.copy_(cur[1]); dB.copy_(cur[2])  # producers of every input, same stream, no sync
+        v.encrypt_device(dF, dD, dB, dE)
+        v.decrypt_device(dE, dD, dB, dP)                       # consumes the ciphertext the call before produced
+        v.encrypt_device(dP, dD, dB, dP)                       # ... and its plaintext, in place
+    torch.cuda.synchronize()
+    want = oracle_frames(orc, F2, D2, B2)
+    assert np.array_equal(dE.cpu().numpy(), want)
+    assert np.array_equal(dP.cpu().numpy(), want)
 
 
 def test_device_call_argument_errors(torch_cuda, vb):
