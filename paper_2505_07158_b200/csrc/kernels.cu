@@ -13,7 +13,9 @@
 // followed by a per-byte-column circular shift in the interleaved H x 3W byte
 // matrix, followed by a byte XOR.  Two tiled passes do exactly that:
 //
-//   row pass    : work unit = a block of 4 rows.  Warp-specialised persistent CTAs: a copy warp brings
+//   row pass    : work unit = a block of 4 rows.  Two variants of the same two phases: row_reg_kernel (frames up to 4096
+//                 pixels wide: a block lands in the threads' registers, three to four small CTAs per SM) and
+//                 row_pass_kernel, described here.  Warp-specialised persistent CTAs: a copy warp brings
 //                 blocks in with bulk async copies (TMA, cp.async.bulk) into a ring of stages and sends
 //                 finished blocks out with bulk async stores; the compute warps de-interleave a block
 //                 into three channel planes (already rotated by the whole-chunk part of the distance),

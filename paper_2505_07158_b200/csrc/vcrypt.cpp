@@ -441,7 +441,7 @@ extern "C" const char *vcrypt_describe(void) {
         std::snprintf(buf, sizeof buf,
                       "vcrypt: LHCS sigma=10 rho=28 beta=8/3, RK4 dt=%.3f, whitening N0=%d steps, IR record stride K_m=%d, "
                       "bound u=%llu, 6 mantissa bytes per variable; host: sha_ni=%d lanes_isa=%d (0 scalar, 1 avx2x4, 2 avx512x8); "
-                      "device: sm_100a warp-specialised TMA row pass + TMA-tensor T4 column pass (PDL-chained), any-shape gather",
+                      "device: sm_100a row pass (register-landing, or TMA-staged warp-specialised) + TMA-tensor T4 column pass (PDL-chained), any-shape gather",
                       vh::kDt, vh::kWhiten, vh::kRecordStride, (unsigned long long)vh::kBound, (int)vh::cpu_has_shani(),
                       vh::best_isa());
         done = true;
