@@ -118,6 +118,33 @@ def test_hash_and_derivation_match_oracle(orc, w, h, n, flags):
     assert k == 3 and np.array_equal(s, oc.state)
 
 
+@pytest.mark.parametrize("flags", [0, vb.FLAG_HOST_SCALAR])
+def test_host_derivation_reproduces_frozen_vector(flags):
+    """tests/golden/derive_tiny.txt (written from oracle/ alone by tests/golden/make_derive_tiny.py and reproduced by the
+    pure-Python restatement in tests/test_oracle_derivation.py): the product's host derivation arrives at the same base
+    states, D and B over the two chained frames without the oracle being involved in this test at all."""
+    import struct
+
+    from conftest import read_golden
+
+    key = (3.141592653589793, 2.718281828459045, 1.4142135623730951, 1.7320508075688772)
+    v = vb.Vcrypt(key, -1.0, 2, 5, 7, flags=HO | flags)
+    rows = read_golden("derive_tiny.txt")
+    nframes = 0
+    for i, row in enumerate(rows):
+        if row[0] != "H":
+            continue
+        S, D, B = rows[i + 1], rows[i + 3], rows[i + 4]
+        assert S[0] == "S" and D[0] == "D" and B[0] == "B"
+        s, k = v.get_state()
+        assert k == nframes and struct.pack("<4d", *s) == struct.pack("<4Q", *[int(x, 16) for x in S[1:]])
+        Dv, Bv = v.derive(bytes.fromhex(row[1]))
+        assert Dv.tolist() == [int(x, 16) for x in D[1:]]
+        assert Bv.tobytes() == bytes.fromhex(B[1])
+        nframes += 1
+    assert nframes == 2
+
+
 def test_lane_paths_agree_on_ragged_worker_slices(orc):
     """n that does not divide h or 3(h+w), and n not a multiple of the lane count: padded lanes, ragged tails,
     and the split into single-lane runs when D iteration counts differ inside a lane group."""

@@ -2,7 +2,10 @@
 reconstruction, D / B layout.  P12 of DESIGN.md: these parts are PARITY UNPINNED against the
 authors' implementation (no vector in the paper); what is checked here is the mathematics -- Eq. (1)
 hand-evaluated, RK4 against a high-accuracy ODE solve, IEEE field invariants, hand-worked
-reconstructions, and the slicing/ordering rules replayed step by step on tiny cases.
+reconstructions -- and the BITS of the readings this repository fixed: a pure-Python binary64
+restatement of SURVEY.md 8(c) steps 2-7 and 10 (py_* below: Python floats and ints only, no numpy
+arithmetic, no call into the oracle) must reproduce the oracle's RK4 states, whitening, IR records, D
+and B bit for bit, and both must reproduce the frozen vector tests/golden/derive_tiny.txt.
 """
 import os
 import struct
@@ -132,20 +135,108 @@ def test_reconstruct_ieee_invariants(orc):
         assert orc.reconstruct(v, bytes(hb2)) != r
 
 
+# ---------------------------------------------------------------------------------------------------
+# Pure-Python binary64 restatement of SURVEY.md 8(c) (PAPER.md:35-43 Eq. 1, :55, :59).  CPython floats are
+# IEEE binary64, every operator below is one correctly rounded operation and nothing can be contracted
+# into an FMA, so the expression order written here IS the arithmetic.  Nothing below calls the oracle.
+# ---------------------------------------------------------------------------------------------------
+DT = 0.005
+HALF_DT = 0.5 * DT
+DT_6 = DT / 6.0
+BETA = 8.0 / 3.0
+K_M, N0, U = 16, 20000, 40
+
+
+def py_f(x, y, z, w, g):
+    """Step 10: f = (10 (y - x) + w, (28 x - y) - x z, x y - (8/3) z, (-(y z)) + gamma w)."""
+    return (10.0 * (y - x) + w, (28.0 * x - y) - x * z, x * y - BETA * z, (-(y * z)) + g * w)
+
+
+def py_rk4_step(s, g):
+    """Step 10: k1 = f(s), k2 = f(s + (dt/2) k1), k3 = f(s + (dt/2) k2), k4 = f(s + dt k3),
+    s' = s + (dt/6) (((k1 + 2 k2) + 2 k3) + k4)."""
+    k1 = py_f(s[0], s[1], s[2], s[3], g)
+    k2 = py_f(s[0] + HALF_DT * k1[0], s[1] + HALF_DT * k1[1], s[2] + HALF_DT * k1[2], s[3] + HALF_DT * k1[3], g)
+    k3 = py_f(s[0] + HALF_DT * k2[0], s[1] + HALF_DT * k2[1], s[2] + HALF_DT * k2[2], s[3] + HALF_DT * k2[3], g)
+    k4 = py_f(s[0] + DT * k3[0], s[1] + DT * k3[1], s[2] + DT * k3[2], s[3] + DT * k3[3], g)
+    return tuple(s[i] + DT_6 * (((k1[i] + 2.0 * k2[i]) + 2.0 * k3[i]) + k4[i]) for i in range(4))
+
+
+def py_rk4(s, g, steps):
+    s = tuple(float(v) for v in s)
+    for _ in range(steps):
+        s = py_rk4_step(s, g)
+    return s
+
+
+def py_reconstruct(v, hb):
+    """Step 3: a = |v|, ip = floor(a), fr = a - ip; I = ((ip & 0xFFFF) ^ (hb0 | hb1 << 8)) mod u;
+    the IEEE pattern of fr XOR the 48-bit little-endian integer hb2..hb7; v' = I + that double."""
+    a = abs(v)
+    ip = int(a)  # truncation = floor for a >= 0
+    fr = a - float(ip)
+    integer = ((ip & 0xFFFF) ^ (hb[0] | hb[1] << 8)) % U
+    bits = struct.unpack("<Q", struct.pack("<d", fr))[0] ^ int.from_bytes(hb[2:8], "little")
+    return float(integer) + struct.unpack("<d", struct.pack("<Q", bits))[0]
+
+
+def _bits(vals):
+    return struct.pack("<%dd" % len(vals), *[float(v) for v in vals])
+
+
+def test_rk4_bits_match_pure_python_restatement(orc):
+    """The 48 low mantissa bits of every iterate ARE the keystream: the oracle's RK4 must be the
+    operation sequence of step 10 bit for bit -- 24 random states and gammas x 1500 steps, compared after every
+    step for the first 50 and at the end.  A re-associated final sum, a fused multiply-add, dt/6 computed as
+    dt * (1/6), or 8/3 written as 2.6666666666666665 +- 1 ulp all fail here."""
+    rng = np.random.default_rng(2024)
+    for _ in range(24):
+        s = tuple(float(v) for v in rng.uniform(-25, 25, 4))
+        g = float(rng.uniform(-1.52, -0.06))
+        o, p = np.array(s), s
+        for _k in range(50):
+            o, p = orc.rk4(o, g, 1), py_rk4_step(p, g)
+            assert _bits(o) == _bits(p)
+        assert _bits(orc.rk4(s, g, 1500)) == _bits(py_rk4(s, g, 1500))
+
+
+def test_single_rhs_and_constants_bits(orc):
+    """Eq. 1's right-hand side alone, bit for bit, and the three rounded constants of step 10."""
+    assert DT_6 == 0.005 / 6.0 and HALF_DT == 0.0025 and struct.pack(">d", BETA).hex() == "4005555555555555"
+    rng = np.random.default_rng(7)
+    for _ in range(200):
+        s = [float(v) for v in rng.uniform(-60, 60, 4)]
+        g = float(rng.uniform(-1.52, -0.06))
+        assert _bits(orc.lhcs_rhs(s, g)) == _bits(py_f(*s, g))
+
+
+def test_whitening_bits_match_pure_python_restatement(orc):
+    """Step 2 / reading Q5: orc_init's base state = the key after N0 = 20000 steps of step 10, bit for bit."""
+    for g, key in ((-1.0, KEY), (-0.06, (1.0, 2.0, 3.0, 4.0)), (-1.52, (-7.25, 0.001, 30.5, -12.0))):
+        assert _bits(orc.ctx(key, g, 2, 4, 4).state) == _bits(py_rk4(key, g, N0))
+
+
+def test_reconstruct_bits_match_pure_python_restatement(orc):
+    rng = np.random.default_rng(11)
+    for _ in range(3000):
+        v = float(rng.uniform(-400, 400))
+        hb = rng.integers(0, 256, 8, dtype=np.uint8).tobytes()
+        assert _bits([orc.reconstruct(v, hb)]) == _bits([py_reconstruct(v, hb)])
+
+
 def _six(d):
     return struct.pack("<d", d)[:6]
 
 
-def replay_derive(orc, S, gamma, n, w, h, H):
-    """Steps 3-7 of DESIGN.md's oracle definition replayed in Python on top of the oracle's own
-    rk4/reconstruct primitives: checks the slicing, skewed fetch, D-before-B order and layouts."""
-    KM = 16
+def replay_derive(S, gamma, n, w, h, H):
+    """Steps 3-7 of SURVEY.md 8(c) replayed on the pure-Python restatement above (none of the oracle's
+    primitives): reconstruction, LHCS_m records, skewed fetch, slicing, D-before-B order and layouts."""
     L = 2 * n
-    s = np.array([orc.reconstruct(S[v], H[8 * v:8 * v + 8]) for v in range(4)])
+    s = tuple(py_reconstruct(float(S[v]), H[8 * v:8 * v + 8]) for v in range(4))
     IR = []
     for g in range(L):
-        s = orc.rk4(s, gamma, KM)
-        IR.append(s.copy())
+        s = py_rk4(s, gamma, K_M)
+        IR.append(s)
     ND = 3 * (h + w)
     D = np.zeros(ND, np.uint16)
     B = np.zeros(3 * w * h, np.uint8)
@@ -153,13 +244,13 @@ def replay_derive(orc, S, gamma, n, w, h, H):
         sys = []
         for q in range(2):
             g = 2 * m + q
-            sys.append(np.array([IR[g][0], IR[(g + 1) % L][1], IR[(g + 2) % L][2], IR[(g + 3) % L][3]]))
+            sys.append((IR[g][0], IR[(g + 1) % L][1], IR[(g + 2) % L][2], IR[(g + 3) % L][3]))
         d0, d1 = m * ND // n, (m + 1) * ND // n
         b0, b1 = (m * h // n) * w * 3, ((m + 1) * h // n) * w * 3
 
         def nxt():
-            sys[0] = orc.rk4(sys[0], gamma, 1)
-            sys[1] = orc.rk4(sys[1], gamma, 1)
+            sys[0] = py_rk4_step(sys[0], gamma)
+            sys[1] = py_rk4_step(sys[1], gamma)
             e0 = b"".join(_six(v) for v in sys[0])
             e1 = b"".join(_six(v) for v in sys[1])
             return bytes(a ^ b for a, b in zip(e0, e1))
@@ -179,16 +270,49 @@ def replay_derive(orc, S, gamma, n, w, h, H):
 def test_derive_layout_replay(orc, n, w, h):
     ctx = orc.ctx(KEY, -1.0, n, w, h)
     S0 = ctx.state
-    assert (S0 == orc.rk4(KEY, -1.0, 20000)).all()  # N0 whitening steps at init
+    assert _bits(S0) == _bits(py_rk4(KEY, -1.0, N0))  # N0 whitening steps at init
     rng = np.random.default_rng(n)
     for frame in range(2):
         H = rng.integers(0, 256, 32, dtype=np.uint8).tobytes()
         S = ctx.state
         D, B, IR = ctx.derive(H, want_ir=True)
-        D2, B2, IR2 = replay_derive(orc, S, -1.0, n, w, h, H)
-        assert (IR == IR2).all()
+        D2, B2, IR2 = replay_derive(S, -1.0, n, w, h, H)
+        assert IR.tobytes() == IR2.tobytes()
         assert (D == D2).all() and (B == B2).all()
-        assert (ctx.state == IR[-1]).all()  # x_2n..w_2n carried to the next frame
+        assert ctx.state.tobytes() == IR[-1].tobytes()  # x_2n..w_2n carried to the next frame
+
+
+def _golden_derive_tiny():
+    frames, cur = [], None
+    for row in read_golden("derive_tiny.txt"):
+        if row[0] == "H":
+            cur = {"H": bytes.fromhex(row[1])}
+            frames.append(cur)
+        elif row[0] in ("S", "IR"):
+            cur[row[0]] = struct.pack("<%dQ" % (len(row) - 1), *[int(x, 16) for x in row[1:]])
+        elif row[0] == "D":
+            cur["D"] = np.array([int(x, 16) for x in row[1:]], np.uint16)
+        elif row[0] == "B":
+            cur["B"] = np.frombuffer(bytes.fromhex(row[1]), np.uint8)
+    return frames
+
+
+def test_golden_derive_tiny_reproduced_by_oracle_and_by_restatement(orc):
+    """tests/golden/derive_tiny.txt (n = 2, 5 x 7, two chained frames; written by tests/golden/make_derive_tiny.py
+    from oracle/ alone): today's oracle still writes these bytes, and the pure-Python restatement -- started from
+    the KEY, not from anything in the file -- arrives at the same base states, IR, D and B."""
+    n, w, h, gamma = 2, 5, 7, -1.0
+    frames = _golden_derive_tiny()
+    assert len(frames) == 2 and frames[0]["D"].size == 3 * (h + w) and frames[0]["B"].size == 3 * w * h
+    ctx = orc.ctx(KEY, gamma, n, w, h)
+    S = py_rk4(KEY, gamma, N0)
+    for fr in frames:
+        assert ctx.state.tobytes() == fr["S"] == _bits(S)
+        D, B, IR = ctx.derive(fr["H"], want_ir=True)
+        assert IR.tobytes() == fr["IR"] and (D == fr["D"]).all() and (B.ravel() == fr["B"]).all()
+        D2, B2, IR2 = replay_derive(S, gamma, n, w, h, fr["H"])
+        assert IR2.tobytes() == fr["IR"] and (D2 == fr["D"]).all() and (B2.ravel() == fr["B"]).all()
+        S = tuple(IR2[-1])
 
 
 def test_worker_streams_are_not_shifted_copies(orc):
