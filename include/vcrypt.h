@@ -53,6 +53,7 @@ extern "C" {
 #define VCRYPT_E_CUDA (-4)   /* CUDA error, or GPU call on a host-only context       */
 #define VCRYPT_E_NOMEM (-5)  /* host or device allocation failed                     */
 #define VCRYPT_E_STATE (-6)  /* chaotic state left the finite range                  */
+#define VCRYPT_E_LIMIT (-7)  /* n above VCRYPT_NOALLOC_MAX_FRAMES in a *_noalloc call    */
 
 /* vcrypt_params.flags */
 #define VCRYPT_FLAG_HOST_ONLY 1u      /* no CUDA: host derivation hooks only (tests on CPU boxes)  */
@@ -206,6 +207,38 @@ int vcrypt_frame_stats_device(vcrypt_ctx *ctx, const void *d_frames, size_t n, v
  * npcr_out, uaci_out: host, n x 4 doubles = {all three channels together, channel 0, 1, 2}. */
 int vcrypt_npcr_uaci_device(vcrypt_ctx *ctx, const void *d_a, const void *d_b, size_t n, double *npcr_out, double *uaci_out,
                             void *cuda_stream);
+
+/* NPCR / UACI (Eq. 14-16) for callers that cannot allocate GPU memory.  Same arguments, same
+ * numbers as vcrypt_npcr_uaci_device; the difference is where the per-frame accumulators live.
+ *
+ * Who this is for.  vcrypt_npcr_uaci_device calls cudaMalloc / cudaFree for its accumulators on every call.  That is
+ * not possible, or not acceptable, for some users of a frame cipher:
+ *   - a process whose HBM has been handed out in full at start-up (an inference server or a framework memory pool that
+ *     reserves the device up front): cudaMalloc simply fails there, however small the request;
+ *   - a capture / encode / encrypt loop with a frame deadline: cudaMalloc and cudaFree take a driver lock and
+ *     cudaFree waits for the whole device, so one call can stall every other stream for an unbounded time;
+ *   - code that runs under a rule of "no allocation after initialisation" (safety-oriented or long-running services
+ *     that must not fragment or fail for lack of memory days into a run).
+ * Such callers use this entry point: it calls no cudaMalloc, cudaFree, cudaMallocAsync or any other allocating routine,
+ * on the device or on the host heap.  The accumulators are a fixed array compiled into libvcrypt.so.
+ *
+ * The price, and the rules:
+ *   - Capacity is fixed: n <= VCRYPT_NOALLOC_MAX_FRAMES (512) per call.  A larger n is refused with VCRYPT_E_LIMIT
+ *     before anything is enqueued (vcrypt_last_cuda_error then says how many were asked for); split the clip.
+ *   - The array (24 KB) occupies memory on EVERY GPU the process uses this library on, from the time the library's
+ *     device code is loaded there until the process exits, also if this function is never called.
+ *   - Set-up on first use: the first call on a given device looks up where that device put the array and remembers it.
+ *     Make that first call during initialisation, outside any stream capture and before timing-critical work; later
+ *     calls on that device only read the remembered address.
+ *   - One array per device is shared by all contexts, streams and threads.  A call zeroes the part it uses (in stream
+ *     order, ahead of its kernel), so leftovers of earlier calls never leak into a result.  But two calls whose GPU
+ *     work may run at the same time on one device -- from two host threads, or on two streams -- race on the array
+ *     and return wrong numbers without any error.  Serialise them (the call itself waits for `cuda_stream` before it
+ *     returns, so calls made one after another from one thread never overlap).
+ * d_a, d_b: device, n x H x W x 3; npcr_out, uaci_out: host, n x 4 doubles, laid out as in vcrypt_npcr_uaci_device. */
+#define VCRYPT_NOALLOC_MAX_FRAMES 512u
+int vcrypt_npcr_uaci_device_noalloc(vcrypt_ctx *ctx, const void *d_a, const void *d_b, size_t n, double *npcr_out,
+                                    double *uaci_out, void *cuda_stream);
 
 /* Local Shannon entropy (Eq. 11): mean over k square blocks (side x side pixels, top-left pixel
  * (x, y) = blocks_xy[2b], blocks_xy[2b+1], chosen by the caller: non-overlapping, inside the frame) of the entropy of

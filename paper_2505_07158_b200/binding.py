@@ -13,7 +13,8 @@ import numpy as np
 
 from . import build as _build
 
-OK, E_ARG, E_KEY, E_SHAPE, E_CUDA, E_NOMEM, E_STATE = 0, -1, -2, -3, -4, -5, -6
+OK, E_ARG, E_KEY, E_SHAPE, E_CUDA, E_NOMEM, E_STATE, E_LIMIT = 0, -1, -2, -3, -4, -5, -6, -7
+NOALLOC_MAX_FRAMES = 512  # VCRYPT_NOALLOC_MAX_FRAMES
 FLAG_HOST_ONLY, FLAG_FORCE_GENERIC, FLAG_HOST_SCALAR, FLAG_DEVICE_DERIVE, FLAG_DEVICE_HASH, FLAG_PERSISTENT, FLAG_ROW_TMA = 1, 2, 4, 8, 16, 32, 64
 
 
@@ -77,6 +78,7 @@ def lib() -> C.CDLL:
     L.vcrypt_frame_hash_device.argtypes = [_vp, _vp, C.c_size_t, _vp, _vp]
     L.vcrypt_frame_stats_device.argtypes = [_vp, _vp, C.c_size_t, C.POINTER(FrameStats), _vp, _vp]
     L.vcrypt_npcr_uaci_device.argtypes = [_vp, _vp, _vp, C.c_size_t, _vp, _vp, _vp]
+    L.vcrypt_npcr_uaci_device_noalloc.argtypes = [_vp, _vp, _vp, C.c_size_t, _vp, _vp, _vp]
     L.vcrypt_local_entropy_device.argtypes = [_vp, _vp, C.c_size_t, _vp, C.c_uint32, C.c_uint32, _vp, _vp]
     _lib = L
     return L
@@ -144,7 +146,7 @@ class Vcrypt:
 
     def _check(self, rc: int, what: str):
         if rc != OK:
-            raise VcryptError(rc, what, self.L.vcrypt_last_cuda_error(self._p).decode() if rc == E_CUDA else "")
+            raise VcryptError(rc, what, self.L.vcrypt_last_cuda_error(self._p).decode() if rc in (E_CUDA, E_LIMIT) else "")
 
     # -- host-buffer calls ---------------------------------------------------------------------------
     def encrypt_frames(self, frames, cipher_out=None, hashes_out=None):
@@ -262,6 +264,19 @@ class Vcrypt:
         self._check(self.L.vcrypt_npcr_uaci_device(self._p, _dev_ptr(d_a, n * self.frame_bytes, "d_a"),
                                                    _dev_ptr(d_b, n * self.frame_bytes, "d_b"), n, npcr.ctypes.data, uaci.ctypes.data,
                                                    0 if stream is None else int(stream)), "vcrypt_npcr_uaci_device")
+        return npcr, uaci
+
+    def npcr_uaci_device_noalloc(self, d_a, d_b, stream=None):
+        """vcrypt_npcr_uaci_device_noalloc -> (npcr, uaci) like npcr_uaci_device, for processes that may not allocate GPU
+        memory (all of it reserved by a pool, a frame deadline, a no-allocation-after-start rule): the accumulators are a
+        fixed array inside libvcrypt.so.  At most NOALLOC_MAX_FRAMES frames per call (VcryptError E_LIMIT above that); one
+        call at a time per GPU -- concurrent calls share the array and corrupt each other's sums."""
+        n = int(d_a.shape[0])
+        npcr, uaci = np.empty((n, 4)), np.empty((n, 4))
+        self._check(self.L.vcrypt_npcr_uaci_device_noalloc(self._p, _dev_ptr(d_a, n * self.frame_bytes, "d_a"),
+                                                           _dev_ptr(d_b, n * self.frame_bytes, "d_b"), n, npcr.ctypes.data,
+                                                           uaci.ctypes.data, 0 if stream is None else int(stream)),
+                    "vcrypt_npcr_uaci_device_noalloc")
         return npcr, uaci
 
     def local_entropy_device(self, d_frames, blocks_xy, side: int, stream=None):

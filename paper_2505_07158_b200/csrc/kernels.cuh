@@ -124,5 +124,11 @@ cudaError_t stats_device(const Geom &g, const uint8_t *d_frames, size_t n, uint3
 cudaError_t diff_device(const Geom &g, const uint8_t *d_a, const uint8_t *d_b, size_t n, unsigned long long *d_out, cudaStream_t st);
 cudaError_t block_hist_device(const Geom &g, const uint8_t *d_frames, size_t n, const uint32_t *d_xy, uint32_t k, uint32_t side,
                               uint32_t *d_bh, cudaStream_t st);
+//   diff_device_static: diff_device with its accumulators in a static device array of the library (no allocation anywhere on
+//                      the path); results land in h_out (HOST, n x 3 x 2 u64) and the stream has been waited for on return.
+//                      At most kDiffStaticMaxFrames frames per call; calls that overlap on one GPU race (see stats.cu).
+constexpr size_t kDiffStaticMaxFrames = 512;  // 512 x 6 x 8 bytes = 24 KB of every GPU that loads the library
+cudaError_t diff_device_static(const Geom &g, const uint8_t *d_a, const uint8_t *d_b, size_t n, unsigned long long *h_out,
+                               cudaStream_t st);
 
 }  // namespace vk

@@ -9,6 +9,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
+
 #include "kernels.cuh"
 
 namespace vk {
@@ -344,6 +346,77 @@ cudaError_t diff_device(const Geom &g, const uint8_t *d_a, const uint8_t *d_b, s
     if (gx < 1u) gx = 1u;
     diff_kernel<<<dim3(gx, (unsigned)n), 256, 0, st>>>(d_a, d_b, g.frame_bytes, d_out);
     return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// NPCR / UACI for callers that must not allocate device memory (vcrypt_npcr_uaci_device_noalloc in include/vcrypt.h).
+//
+// diff_kernel accumulates into 6 words per frame that have to exist somewhere in global memory and start at zero.
+// diff_device gets them from its caller, who allocated them.  Here they live in the library image instead: a
+// file-scope __device__ array of kDiffStaticMaxFrames x 6 words (24 KB).  Every GPU that loads libvcrypt.so carries
+// its own copy from the moment the module is loaded until the process exits, whether or not this path is ever used.
+//
+// Two things follow from that choice and are the caller's to know:
+//   * `g_diff_acc` below is a DEVICE symbol.  In host code the identifier is only a handle for the runtime; it is not
+//     an address the GPU understands.  The address each device gave its copy is asked for once per device
+//     (cudaGetSymbolAddress, with that device current) and kept in a small table; only that value is handed to
+//     cudaMemsetAsync, to the kernel and to cudaMemcpyAsync.
+//   * There is ONE array per device, shared by every context, stream and thread in the process, and it keeps what the
+//     previous call left in it.  Each call clears the 6n words it is about to use, in stream order, before its kernel.
+//     Two calls whose GPU work can overlap in time (different streams, or different host threads) would clear and add
+//     into the same words: that is a data race with wrong results, not an error the library can detect.
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+
+static __device__ __align__(256) unsigned long long g_diff_acc[kDiffStaticMaxFrames * 6u];
+
+constexpr int kDiffStaticMaxDevices = 64;
+
+// Device address of the current device's copy of g_diff_acc.  The first call on a device performs the lookup (which
+// may also be what makes the runtime load this module onto that device); later calls read the table.
+cudaError_t diff_static_address(unsigned long long **out) {
+    static std::mutex mu;
+    static unsigned long long *table[kDiffStaticMaxDevices] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kDiffStaticMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!table[dev]) {
+        unsigned long long *ptr = nullptr;
+        e = cudaGetSymbolAddress((void **)&ptr, g_diff_acc);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        table[dev] = ptr;
+    }
+    *out = table[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+// Same sums as diff_device, accumulated in the library's own static device array and copied to h_out (host, n x 6 words:
+// per channel the number of differing bytes and the sum of |a - b|).  Calls nothing that allocates or frees device
+// memory.  Waits for the stream before returning, so h_out is complete and the array is free for the next call.
+// n > kDiffStaticMaxFrames: cudaErrorInvalidValue (the C entry point checks first and reports VCRYPT_E_LIMIT).
+cudaError_t diff_device_static(const Geom &g, const uint8_t *d_a, const uint8_t *d_b, size_t n, unsigned long long *h_out,
+                               cudaStream_t st) {
+    if (!n) return cudaSuccess;
+    if (n > kDiffStaticMaxFrames) return cudaErrorInvalidValue;
+    unsigned long long *acc = nullptr;
+    cudaError_t e = diff_static_address(&acc);
+    if (e != cudaSuccess) return e;
+    const size_t bytes = n * 6u * sizeof(unsigned long long);
+    e = cudaMemsetAsync(acc, 0, bytes, st);  // the previous call's sums are still in there
+    if (e != cudaSuccess) return e;
+    uint32_t gx = (uint32_t)((g.frame_bytes / 12u + 256u * 8u - 1u) / (256u * 8u));
+    if (gx > 592u) gx = 592u;
+    if (gx < 1u) gx = 1u;
+    diff_kernel<<<dim3(gx, (unsigned)n), 256, 0, st>>>(d_a, d_b, g.frame_bytes, acc);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_out, acc, bytes, cudaMemcpyDeviceToHost, st);
+    const cudaError_t es = cudaStreamSynchronize(st);  // also after a failure: nothing of this call may still be running
+    return e != cudaSuccess ? e : es;
 }
 
 cudaError_t block_hist_device(const Geom &g, const uint8_t *d_frames, size_t n, const uint32_t *d_xy, uint32_t k, uint32_t side,

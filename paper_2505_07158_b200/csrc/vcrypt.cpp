@@ -430,6 +430,7 @@ extern "C" const char *vcrypt_strerror(int code) {
         case VCRYPT_E_CUDA: return "CUDA error, or GPU call on a host-only context";
         case VCRYPT_E_NOMEM: return "out of memory";
         case VCRYPT_E_STATE: return "chaotic state left the finite range";
+        case VCRYPT_E_LIMIT: return "more frames than the fixed scratch of a no-allocation call holds (VCRYPT_NOALLOC_MAX_FRAMES)";
         default: return "unknown vcrypt error code";
     }
 }
@@ -741,6 +742,42 @@ extern "C" int vcrypt_npcr_uaci_device(vcrypt_ctx *c, const void *d_a, const voi
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (d_out) cudaFree(d_out);
         if (e != cudaSuccess) return cuda_fail(c, e, "NPCR / UACI");
+        const double N = (double)c->g.w * (double)c->g.h;
+        for (size_t f = 0; f < n; ++f) {
+            unsigned long long ne = 0, ad = 0;
+            for (int ch = 0; ch < 3; ++ch) {
+                const unsigned long long a = r[f * 6u + 2 * ch], b = r[f * 6u + 2 * ch + 1];
+                ne += a;
+                ad += b;
+                npcr[4 * f + 1 + ch] = 100.0 * (double)a / N;            // Eq. 14, 16
+                uaci[4 * f + 1 + ch] = 100.0 * (double)b / (N * 255.0);  // Eq. 15
+            }
+            npcr[4 * f] = 100.0 * (double)ne / (3.0 * N);
+            uaci[4 * f] = 100.0 * (double)ad / (3.0 * N * 255.0);
+        }
+        return VCRYPT_OK;
+    });
+}
+
+// The no-allocation twin of vcrypt_npcr_uaci_device (include/vcrypt.h): same sums, same binary64 steps, but the device
+// accumulators are the library's static array (stats.cu) and the host landing buffer is on this thread's stack, so nothing
+// on the path asks CUDA (or the heap) for memory.
+extern "C" int vcrypt_npcr_uaci_device_noalloc(vcrypt_ctx *c, const void *d_a, const void *d_b, size_t n, double *npcr, double *uaci,
+                                               void *stream) {
+    return guarded([&]() -> int {
+        if (!c || !d_a || !d_b || !npcr || !uaci || n == 0) return VCRYPT_E_ARG;
+        if (n > VCRYPT_NOALLOC_MAX_FRAMES) {
+            std::snprintf(c->cuda_msg, sizeof c->cuda_msg, "vcrypt_npcr_uaci_device_noalloc: n = %zu frames, the static scratch holds %u",
+                          n, (unsigned)VCRYPT_NOALLOC_MAX_FRAMES);
+            return VCRYPT_E_LIMIT;
+        }
+        if (!c->cuda) return VCRYPT_E_CUDA;
+        VC_DEVICE(c);
+        static_assert(VCRYPT_NOALLOC_MAX_FRAMES == vk::kDiffStaticMaxFrames, "header and kernel limits must agree");
+        unsigned long long r[vk::kDiffStaticMaxFrames * 6u];  // 24 KB of stack
+        const cudaError_t e = vk::diff_device_static(c->g, static_cast<const uint8_t *>(d_a), static_cast<const uint8_t *>(d_b), n, r,
+                                                     static_cast<cudaStream_t>(stream));
+        if (e != cudaSuccess) return cuda_fail(c, e, "NPCR / UACI (static scratch)");
         const double N = (double)c->g.w * (double)c->g.h;
         for (size_t f = 0; f < n; ++f) {
             unsigned long long ne = 0, ad = 0;
