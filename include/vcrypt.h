@@ -88,7 +88,7 @@ typedef struct vcrypt_params {
                                at least 4 x pipe_frames frames; such a call alternates its launch pairs over
                                `pipe_streams` streams (the caller's + internal ones forked from and joined into it),
                                so that one pair's column pass overlaps the next pair's row pass.  0 -> from the frame
-                               size (about 31 MB of frames per pair when encrypting, 37 MB when decrypting).  Does not affect results                     */
+                               size (about 31 MB of frames per pair, in both directions).  Does not affect results                     */
     uint32_t pipe_streams;  /* 0 -> 2; 1 -> off (every launch on the caller's stream); at most 4                    */
     /* tuning of the persistent cipher kernel (0 -> chosen from the frame size); none of them affects results */
     uint32_t tune_row_stages;      /* input stages of the row team's shared-memory ring                            */

@@ -32,7 +32,7 @@ CXX_SOURCES = [
     ("host_lhcs_avx2.cpp", ["-mavx2", "-mclflushopt"]),
     ("host_lhcs_avx512.cpp", ["-mavx512f", "-mavx512dq", "-mprefer-vector-width=512", "-mclflushopt"]),
 ]
-HEADERS = ["host.hpp", "kernels.cuh", "ptx.cuh", "thread_pool.hpp", "host_lhcs_lanes.inc", os.path.join("..", "..", "include", "vcrypt.h")]
+HEADERS = ["host.hpp", "kernels.cuh", "ptx.cuh", "smem_attr.hpp", "thread_pool.hpp", "host_lhcs_lanes.inc", os.path.join("..", "..", "include", "vcrypt.h")]
 
 
 def _nvcc() -> str:

@@ -44,6 +44,7 @@
 
 #include "kernels.cuh"
 #include "ptx.cuh"
+#include "smem_attr.hpp"
 
 namespace vk {
 
@@ -813,8 +814,8 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 template <bool INV, int X, int NSW_>
-static cudaError_t uni_attr(size_t smem) {
-    return cudaFuncSetAttribute(cipher_kernel<INV, X, NSW_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+static cudaError_t uni_attr(int device, size_t smem) {
+    return raise_dyn_smem((const void *)cipher_kernel<INV, X, NSW_>, device, smem);
 }
 
 cudaError_t make_uni_plan(const Geom &g, int device, const UniTune &tune, UniPlan *out) {
@@ -872,8 +873,8 @@ cudaError_t make_uni_plan(const Geom &g, int device, const UniTune &tune, UniPla
             if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
                 qres == cudaDriverEntryPointSuccess && fn) {
                 p.encode_tiled = fn;
-                if (X == 64) { e = uni_attr<false, 64, NSW>(p.smem); if (!e) e = uni_attr<true, 64, NSW>(p.smem); }
-                else { e = uni_attr<false, 32, NSW>(p.smem); if (!e) e = uni_attr<true, 32, NSW>(p.smem); }
+                if (X == 64) { e = uni_attr<false, 64, NSW>(device, p.smem); if (!e) e = uni_attr<true, 64, NSW>(device, p.smem); }
+                else { e = uni_attr<false, 32, NSW>(device, p.smem); if (!e) e = uni_attr<true, 32, NSW>(device, p.smem); }
                 if (e != cudaSuccess) return e;
                 p.ok = true;
             }

@@ -47,6 +47,7 @@ struct WorkerSlice {
 // 2 AVX-512 (8 lanes).  Every isa produces the same bytes.  Returns false on a non-finite state.
 bool derive_workers(const WorkerSlice *ws, size_t count, double gamma, int isa);
 int best_isa();  // what this CPU supports
+bool has_clflushopt();  // CPUID leaf 7 EBX bit 23 (the lane code flushes finished keystream slices only where this holds)
 
 bool derive_workers_scalar(const WorkerSlice *ws, size_t count, double gamma);
 bool derive_workers_avx2(const WorkerSlice *ws, size_t count, double gamma);

@@ -3,6 +3,9 @@
 // (Algorithm 1 steps 7-13) and the split of a frame's D / B into worker slices (Algorithm 2,
 // PAPER.md:88-110).  Must be compiled with -ffp-contract=off (no FMA contraction): the expression order below
 // is the arithmetic.  Shares nothing with oracle/.
+#if defined(__x86_64__)
+#include <cpuid.h>
+#endif
 #include "host.hpp"
 
 #include <cmath>
@@ -106,6 +109,20 @@ int best_isa() {
     return v;
 #else
     return 0;
+#endif
+}
+
+// CLFLUSHOPT is its own CPUID bit (leaf 7, sub-leaf 0, EBX bit 23), not implied by AVX2: Haswell and Broadwell have AVX2
+// without it, and the lane code's flush (host_lhcs_lanes.inc) would be an illegal instruction there.
+bool has_clflushopt() {
+#if defined(__x86_64__)
+    static const bool v = [] {
+        unsigned a = 0, b = 0, c = 0, d = 0;
+        return __get_cpuid_count(7, 0, &a, &b, &c, &d) != 0 && ((b >> 23) & 1u) != 0;
+    }();
+    return v;
+#else
+    return false;
 #endif
 }
 

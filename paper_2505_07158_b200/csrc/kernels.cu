@@ -45,6 +45,7 @@
 
 #include "kernels.cuh"
 #include "ptx.cuh"
+#include "smem_attr.hpp"
 
 namespace vk {
 
@@ -440,9 +441,12 @@ __global__ void __launch_bounds__(NT, MINB) row_reg_kernel(const uint8_t *src, u
 // columns x four byte lanes) and a sub-warp emits groups of 8 consecutive output rows with 64-bit
 // keystream loads and ciphertext stores.  Bank of a load = (strip row * X/4 + word column) mod 32 with strip
 // row = 4R + b: sub-warp s walks its columns in the order (word column a_l ^ (s & 1), byte lane a_b ^ (s >> 1)),
-// so the sub-warps of a warp always sit in disjoint banks whatever rows they read: no conflicts for
-// X = 128, 64, 32.  The permutation is undone by the selectors of the 4 x 4 byte transposes and by one
-// select per output word.
+// so the sub-warps of a warp sit in disjoint banks whatever rows they read -- that is the design intent for the GATHER
+// loads at X = 128, 64, 32.  It does not make the kernel conflict-free: the round-2 full capture
+// (profiles/r2_ncu_full_summary.csv) counts 185 K bank-conflict wavefronts out of 572 K shared-memory wavefronts per
+// launch of col_enc_kernel<64,256,2,2>, i.e. about half as many again as a conflict-free kernel would issue; which
+// instruction they belong to has not been attributed (no source-level capture yet).  The permutation is undone by the
+// selectors of the 4 x 4 byte transposes and by one select per output word.
 // In place is safe: the whole strip is in shared memory before the first store.
 // ---------------------------------------------------------------------------------------------
 // keystream prefetch depths (rounds of loads in flight per thread): decrypt column pass with three CTAs per SM / one CTA per
@@ -954,12 +958,12 @@ static size_t rowreg_smem_bytes(const Geom &g) { return (size_t)RR_HDR + (size_t
 static size_t cole_smem_bytes(const Geom &g, int X) { return (size_t)(g.h + CE_PAD) * X + 16 + 2 * (size_t)X; }
 
 template <int X, int NT, int MINB, int KD>
-static cudaError_t col_set_attr(size_t smem) {
-    return cudaFuncSetAttribute(col_dec_kernel<X, NT, MINB, KD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+static cudaError_t col_set_attr(int device, size_t smem) {
+    return raise_dyn_smem((const void *)col_dec_kernel<X, NT, MINB, KD>, device, smem);
 }
 template <int X, int NT, int MINB, int DEPTH>
-static cudaError_t cole_set_attr(size_t smem) {
-    return cudaFuncSetAttribute(col_enc_kernel<X, NT, MINB, DEPTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+static cudaError_t cole_set_attr(int device, size_t smem) {
+    return raise_dyn_smem((const void *)col_enc_kernel<X, NT, MINB, DEPTH>, device, smem);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -1083,24 +1087,24 @@ cudaError_t make_plan(const Geom &g, int device, bool row_tma, Plan *out) {
             const size_t l2_budget = (size_t)100 << 20;
             p.max_frames_per_launch = l2_budget / g.frame_bytes ? l2_budget / g.frame_bytes : 1;
             if (ctas == 3) {
-                if (X == 64) { e = col_set_attr<64, 256, 3, VK_KD3>(p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3, 1>(p.smem_cole_enc); if (!e) e = cole_set_attr<64, 256, 2, VK_DE2>(p.smem_cole_enc); }
-                else { e = col_set_attr<32, 256, 3, VK_KD3>(p.smem_cole); if (!e) e = cole_set_attr<32, 256, 3, 1>(p.smem_cole_enc); }
+                if (X == 64) { e = col_set_attr<64, 256, 3, VK_KD3>(device, p.smem_cole); if (!e) e = cole_set_attr<64, 256, 3, 1>(device, p.smem_cole_enc); if (!e) e = cole_set_attr<64, 256, 2, VK_DE2>(device, p.smem_cole_enc); }
+                else { e = col_set_attr<32, 256, 3, VK_KD3>(device, p.smem_cole); if (!e) e = cole_set_attr<32, 256, 3, 1>(device, p.smem_cole_enc); }
             } else {
-                if (X == 64) { e = col_set_attr<64, 512, 1, VK_KD1>(p.smem_cole); if (!e) e = cole_set_attr<64, 512, 1, VK_DE1>(p.smem_cole_enc); }
-                else { e = col_set_attr<32, 512, 1, VK_KD1>(p.smem_cole); if (!e) e = cole_set_attr<32, 512, 1, VK_DE1>(p.smem_cole_enc); }
+                if (X == 64) { e = col_set_attr<64, 512, 1, VK_KD1>(device, p.smem_cole); if (!e) e = cole_set_attr<64, 512, 1, VK_DE1>(device, p.smem_cole_enc); }
+                else { e = col_set_attr<32, 512, 1, VK_KD1>(device, p.smem_cole); if (!e) e = cole_set_attr<32, 512, 1, VK_DE1>(device, p.smem_cole_enc); }
             }
             if (e != cudaSuccess) return e;
-            e = cudaFuncSetAttribute(row_pass_kernel<false, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
-            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
-            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_dec);
-            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<false, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
-            if (!e) e = cudaFuncSetAttribute(row_pass_kernel<true, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row);
-            if (!e && p.row_reg == 1) e = cudaFuncSetAttribute(row_reg_kernel<false, 256, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
-            if (!e && p.row_reg == 1) e = cudaFuncSetAttribute(row_reg_kernel<true, 256, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
-            if (!e && p.row_reg == 2) e = cudaFuncSetAttribute(row_reg_kernel<false, 512, 3, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
-            if (!e && p.row_reg == 2) e = cudaFuncSetAttribute(row_reg_kernel<true, 512, 3, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
-            if (!e && p.row_reg == 3) e = cudaFuncSetAttribute(row_reg_kernel<false, 512, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
-            if (!e && p.row_reg == 3) e = cudaFuncSetAttribute(row_reg_kernel<true, 512, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_row_reg);
+            e = raise_dyn_smem((const void *)row_pass_kernel<false, 512, 2>, device, p.smem_row);
+            if (!e) e = raise_dyn_smem((const void *)row_pass_kernel<true, 512, 2>, device, p.smem_row);
+            if (!e) e = raise_dyn_smem((const void *)row_pass_kernel<true, 256, 3>, device, p.smem_row_dec);
+            if (!e) e = raise_dyn_smem((const void *)row_pass_kernel<false, 1024, 1>, device, p.smem_row);
+            if (!e) e = raise_dyn_smem((const void *)row_pass_kernel<true, 1024, 1>, device, p.smem_row);
+            if (!e && p.row_reg == 1) e = raise_dyn_smem((const void *)row_reg_kernel<false, 256, 4, 1>, device, p.smem_row_reg);
+            if (!e && p.row_reg == 1) e = raise_dyn_smem((const void *)row_reg_kernel<true, 256, 4, 1>, device, p.smem_row_reg);
+            if (!e && p.row_reg == 2) e = raise_dyn_smem((const void *)row_reg_kernel<false, 512, 3, 1>, device, p.smem_row_reg);
+            if (!e && p.row_reg == 2) e = raise_dyn_smem((const void *)row_reg_kernel<true, 512, 3, 1>, device, p.smem_row_reg);
+            if (!e && p.row_reg == 3) e = raise_dyn_smem((const void *)row_reg_kernel<false, 512, 2, 2>, device, p.smem_row_reg);
+            if (!e && p.row_reg == 3) e = raise_dyn_smem((const void *)row_reg_kernel<true, 512, 2, 2>, device, p.smem_row_reg);
             if (e != cudaSuccess) return e;
         }
     }

@@ -34,7 +34,7 @@ struct Plan {
     size_t smem_row_dec;
     int row_reg;           // register-landing row pass (row_reg_kernel): 0 = not used, 1 = 256-thread CTAs (w <= 1024), 2 = 512-thread
                            // CTAs (w <= 2048), 3 = 512-thread CTAs with two items per thread (w <= 4096)
-    bool row_reg_dec;      // ... also for the inverse row pass (wide frames only: measured)
+    bool row_reg_dec;      // ... also for the inverse row pass (every width except 1537 - 2048 pixels: measured, see make_plan)
     int row_reg_grid_max;  // its persistent CTAs
     size_t smem_row_reg;
     uint32_t box_rows;     // column pass: rows per TMA tensor tile (largest divisor of h that is <= 256)

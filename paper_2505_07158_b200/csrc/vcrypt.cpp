@@ -227,8 +227,18 @@ int retire_slot(vcrypt_ctx *c, Slot &s) {
 int sched_for_stream(vcrypt_ctx *c, cudaStream_t st, uint32_t **out) {
     const size_t words = vk::cipher_sched_words(vcrypt_ctx::kSchedFrames);
     if (!c->d_sched) {
-        VC_CUDA(c, cudaMalloc(&c->d_sched, vcrypt_ctx::kSchedSlots * words * sizeof(uint32_t)));
-        VC_CUDA(c, cudaMemset(c->d_sched, 0, vcrypt_ctx::kSchedSlots * words * sizeof(uint32_t)));
+        // One-time zeroing.  cudaMemset of device memory is asynchronous to the host and runs on the legacy default stream, which
+        // does not order it before work on a non-blocking stream (the library's own slot streams, torch's, cupy's): the first
+        // launch on `st` could read the ticket and the per-frame counters before they are zero.  So the host waits for it here.
+        uint32_t *buf = nullptr;
+        VC_CUDA(c, cudaMalloc(&buf, vcrypt_ctx::kSchedSlots * words * sizeof(uint32_t)));
+        cudaError_t e = cudaMemset(buf, 0, vcrypt_ctx::kSchedSlots * words * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaStreamSynchronize(cudaStreamLegacy);
+        if (e != cudaSuccess) {  // not kept: a buffer that is allocated but not known to be zero must never be handed out
+            cudaFree(buf);
+            return cuda_fail(c, e, "zeroing the persistent kernel's launch state");
+        }
+        c->d_sched = buf;
     }
     for (int i = 0; i < c->sched_n; ++i)
         if (c->sched_owner[i] == st) { *out = c->d_sched + (size_t)i * words; return VCRYPT_OK; }
@@ -523,7 +533,8 @@ int derive_frames(vcrypt_ctx *c, double S[4], const uint8_t *hashes, size_t m, u
     }
     // a batch whose keystream would stay in the cores' private caches (single-frame calls: latency) is flushed by the jobs
     // that write it; a large batch spills to memory by itself and the flushes would only cost the host-bound pipeline time
-    if (flush_B && m * c->g.frame_bytes <= ((size_t)32 << 20))
+    // (only on CPUs that have CLFLUSHOPT: the AVX2 / AVX-512 units are compiled with it, AVX2 alone does not imply it)
+    if (flush_B && vh::has_clflushopt() && m * c->g.frame_bytes <= ((size_t)32 << 20))
         for (size_t i = 0; i < m * n; ++i) c->slices[i].flush_B = true;
     const int isa = c->isa;
     const size_t lanes = isa == 2 ? 8 : isa == 1 ? 4 : 1;
