@@ -5,9 +5,9 @@ Kernel level  : vcrypt_encrypt_device / vcrypt_decrypt_device with random D, B (
                 oracle's literal bit-matrix Algorithms 3-7, over tiled shapes, ragged any-shape cases, special
                 distances and in-place calls.
 Whole path    : vcrypt_encrypt_frames / vcrypt_decrypt_frames (rows a1-a12) against the oracle's Algorithm 1
-                on the BASELINE.json configs, every frame element by element: C1, C2 in full; C3 all 30 frames,
-                C4 100 frames, C5 20 frames at full size in bench's launch configuration, with every hash compared
-                and the round trip checked on every frame.
+                on the BASELINE.json configs, every frame element by element: C1 and C2 in full, and the whole
+                clips of C3 (30 frames), C4 (300 frames) and C5 (120 frames of 4K) at full size in bench's launch
+                configuration, with every hash compared and the round trip checked on every frame.
 """
 import numpy as np
 import pytest
@@ -332,6 +332,43 @@ def test_calls_chained_on_one_stream_without_host_sync(torch_cuda, vb, orc, w, h
     assert np.array_equal(dP.cpu().numpy(), want)
 
 
+def test_two_live_contexts_of_different_shapes(torch_cuda, vb, orc):
+    """The opt-in shared-memory limit of a kernel is state of the FUNCTION in the whole process, not of a context: a large
+    shape's context must keep working after a smaller shape's context (same kernel instantiations, smaller strips and rings)
+    has been created later, in every order and for every kernel family (kernel pairs, TMA-staged row pass, persistent)."""
+    shapes = [(1920, 1080), (640, 480), (1280, 720)]
+    cases = {wh: rnd_case(wh[0], wh[1], 2, seed=sum(wh)) for wh in shapes}
+    want = {wh: oracle_frames(orc, *cases[wh]) for wh in shapes}
+    for flags in (0, vb.FLAG_ROW_TMA, vb.FLAG_PERSISTENT):
+        big = gpu_ctx(vb, 1920, 1080, flags=flags)
+        assert np.array_equal(run_device(torch_cuda, big, *cases[(1920, 1080)]), want[(1920, 1080)])
+        small = gpu_ctx(vb, 640, 480, flags=flags)   # created AFTER the large one: must not lower its limits
+        mid = gpu_ctx(vb, 1280, 720, flags=flags)
+        for _ in range(2):
+            for v, wh in ((big, (1920, 1080)), (small, (640, 480)), (mid, (1280, 720)), (big, (1920, 1080))):
+                E = run_device(torch_cuda, v, *cases[wh])
+                assert np.array_equal(E, want[wh]), (flags, wh)
+                assert np.array_equal(run_device(torch_cuda, v, E, cases[wh][1], cases[wh][2], decrypt=True), cases[wh][0]), (flags, wh)
+
+
+def test_persistent_kernel_first_launch_on_a_non_blocking_stream(torch_cuda, vb, orc):
+    """The persistent kernel's launch state is zeroed once per context; that must have happened before the first launch also
+    when the launch goes to a stream that does not synchronise with the default stream and nothing else precedes it there."""
+    torch = torch_cuda
+    w, h, nf = 640, 480, 6
+    F, D, B = rnd_case(w, h, nf, seed=4242)
+    dF, dD, dB = torch.from_numpy(F).cuda(), torch.from_numpy(D.view(np.int16)).cuda(), torch.from_numpy(B).cuda()
+    dE = torch.empty_like(dF)
+    want = oracle_frames(orc, F, D, B)
+    for _ in range(3):  # a fresh context each time: its very first GPU work is the kernel on the side stream
+        st = torch.cuda.Stream()  # torch's streams are created non-blocking
+        torch.cuda.synchronize()
+        v = gpu_ctx(vb, w, h, flags=vb.FLAG_PERSISTENT)
+        v.encrypt_device(dF, dD, dB, dE, st.cuda_stream)
+        st.synchronize()
+        assert np.array_equal(dE.cpu().numpy(), want)
+
+
 def test_device_call_argument_errors(torch_cuda, vb):
     torch = torch_cuda
     v = gpu_ctx(vb, 64, 48)
@@ -410,31 +447,47 @@ def test_config2_full(vb, orc):
     assert np.array_equal(P, frames)
 
 
-def full_parity(vb, orc, cfg, nframes, pinned):
-    """Full-size config in bench's launch configuration: every hash and every frame's ciphertext element by element
-    against the oracle (its D, B follow the whole chain), round trip on every frame."""
+def full_parity(vb, orc, cfg, nframes, pinned, chunk_batches=3):
+    """Full-size config in bench's launch configuration (batches of cfg.batch frames over cfg.n_streams streams): every hash
+    and every frame's ciphertext element by element against the oracle (its D, B follow the whole chain), round trip on every
+    frame.  The clip is streamed through in chunks of chunk_batches batches -- drawn, encrypted (the context carries the chain
+    from call to call), checked, decrypted, dropped -- so host memory stays bounded at 4K; the oracle's per-frame work (hash,
+    literal bit-matrix confusion) runs on a few host threads, its chain step stays serial."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+
     import torch
 
+    chunk = chunk_batches * cfg.batch
+    shape = (chunk, cfg.h, cfg.w, 3)
     if pinned:
-        tin = torch.empty((nframes, cfg.h, cfg.w, 3), dtype=torch.uint8).pin_memory()
-        frames = synth.video(cfg, nframes, out=tin.numpy())
-        tout = torch.empty_like(tin).pin_memory()
-        C = tout.numpy()
+        tin, tout, tpl = (torch.empty(shape, dtype=torch.uint8).pin_memory() for _ in range(3))
+        fin, C, P = tin.numpy(), tout.numpy(), tpl.numpy()
     else:
-        frames = synth.video(cfg, nframes)
-        C = np.empty_like(frames)
-    Hs = np.empty((nframes, 32), np.uint8)
+        fin, C, P = (np.empty(shape, np.uint8) for _ in range(3))
+    Hs = np.empty((chunk, 32), np.uint8)
     enc = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
-    enc.encrypt_frames(frames, C, Hs)
-    oc = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
-    for k in range(nframes):
-        H = orc.frame_hash(frames[k], synth.N_WORKERS)
-        assert H == Hs[k].tobytes(), k
-        D, B = oc.derive(H)
-        assert np.array_equal(C[k], orc.confuse_xor(frames[k], D, B)), k
     dec = gpu_ctx(vb, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams)
-    P = dec.decrypt_frames(C, Hs)
-    assert np.array_equal(P, frames)
+    oc = orc.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    frames = synth.frame_iter(cfg, nframes)
+    done = 0
+    with ThreadPoolExecutor(max(1, min(8, (os.cpu_count() or 2) - 1))) as pool:
+        while done < nframes:
+            m = min(chunk, nframes - done)
+            for k in range(m):
+                fin[k] = next(frames)
+            enc.encrypt_frames(fin[:m], C[:m], Hs[:m])
+            want_H = list(pool.map(lambda k: orc.frame_hash(fin[k], synth.N_WORKERS), range(m)))
+            DB = []
+            for k in range(m):
+                assert want_H[k] == Hs[k].tobytes(), done + k
+                DB.append(oc.derive(want_H[k]))
+            same = list(pool.map(lambda k: bool(np.array_equal(C[k], orc.confuse_xor(fin[k], *DB[k]))), range(m)))
+            assert all(same), [done + k for k in range(m) if not same[k]]
+            dec.decrypt_frames(C[:m], Hs[:m], P[:m])
+            assert np.array_equal(P[:m], fin[:m]), done
+            done += m
+    assert done == nframes
     return enc
 
 
@@ -444,14 +497,17 @@ def test_config3_fhd_batch1(vb, orc):
 
 
 def test_config4_fhd_batches_of_8_three_streams(vb, orc):
+    """Long test (about a minute): the WHOLE clip of config 4, all 300 frames against the oracle."""
     cfg = synth.CONFIGS["C4"]
-    enc = full_parity(vb, orc, cfg, 100, pinned=True)  # 12 full batches + 4, all 100 frames against the oracle
-    assert enc.launch_count()[1] >= 13
+    enc = full_parity(vb, orc, cfg, cfg.frames, pinned=True)
+    assert cfg.frames == 300 and enc.launch_count()[1] >= 2 * 38  # 37 full batches + 4 frames, a launch pair each
 
 
 def test_config5_4k(vb, orc):
+    """Long test (about two minutes): the WHOLE clip of config 5, all 120 frames of 3840 x 2160 against the oracle."""
     cfg = synth.CONFIGS["C5"]
-    full_parity(vb, orc, cfg, 20, pinned=True)  # all 20 frames
+    full_parity(vb, orc, cfg, cfg.frames, pinned=True)
+    assert cfg.frames == 120
 
 
 def test_config4_one_bit_pairs_npcr_uaci(vb, torch_cuda):
