@@ -118,6 +118,25 @@ def time_oracle(cfg, frames_np, nframes):
     return nframes / dt, C, H
 
 
+def time_oracle_phases(cfg, frames_np, nframes):
+    """ms per frame of the oracle's three phases (the paper's Fig. 13 split): sub-frame hashing,
+    derivation (reconstruction + LHCS_m + worker systems -> D, B) and bit-level confusion + XOR, each timed on its own over the
+    first `nframes` frames, one thread."""
+    O = oracle_lib()
+    oc = O.ctx(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h)
+    t = [0.0, 0.0, 0.0]
+    for k in range(nframes):
+        t0 = time.perf_counter()
+        H = O.frame_hash(frames_np[k], synth.N_WORKERS)
+        t1 = time.perf_counter()
+        D, B = oc.derive(H)
+        t2 = time.perf_counter()
+        O.confuse_xor(frames_np[k], D, B)
+        t3 = time.perf_counter()
+        t[0] += t1 - t0; t[1] += t2 - t1; t[2] += t3 - t2
+    return {"hash": 1e3 * t[0] / nframes, "derivation": 1e3 * t[1] / nframes, "confusion_xor": 1e3 * t[2] / nframes, "frames": nframes}
+
+
 def run_reference(args, cfg):
     """--impl reference: the oracle, as it stands, on the host cores (one thread), bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -167,6 +186,33 @@ def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, sustained
     def clip_step():
         kctx.encrypt_device(d_F, d_D, d_B, d_E, stream)
         return kctx.launch_count()[0]
+
+    if args.kernel_leg_only and args.direction:
+        # one direction only, W untimed + K timed calls on the resident clip: the command the decrypt / 4K captures in profiles/ run
+        d_P = torch.empty_like(d_F)
+        clip_step()  # the ciphertext the decrypt direction reads
+        torch.cuda.synchronize()
+
+        def dir_step():
+            if args.direction == "decrypt":
+                kctx.decrypt_device(d_E, d_D, d_B, d_P, stream)
+            else:
+                kctx.encrypt_device(d_F, d_D, d_B, d_E, stream)
+            return kctx.launch_count()[0]
+
+        for _ in range(W):
+            dir_step()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        n = 0
+        for _ in range(K):
+            n += dir_step()
+        e1.record()
+        barrier()
+        ok = bool(torch.equal(d_P, d_F)) if args.direction == "decrypt" else True
+        kctx.destroy()
+        return {"direction": args.direction, "total_ms": e0.elapsed_time(e1), "launches": n, "warm_steps": W, "ok": ok}
 
     def batch_step():
         n = 0
@@ -218,6 +264,50 @@ def kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, sustained
     out["batches_steps"] = KB
     out["batches_launches_per_step"] = bl // KB
     out["batches_same"] = bool(synth.digest(d_E.cpu().numpy()) == out["digest_all"])
+
+    # config 4 as BASELINE.json words it, literally: batches of cfg.batch frames per call, round-robin over cfg.n_streams CALLER
+    # streams (one context per stream: a context belongs to one caller), forked from and joined into the timing stream by events
+    ns = max(1, cfg.n_streams)
+    side = [torch.cuda.Stream() for _ in range(ns)]
+    sctx = [vb.Vcrypt(synth.KEY, synth.GAMMA, synth.N_WORKERS, cfg.w, cfg.h, batch=cfg.batch, n_streams=cfg.n_streams, host_threads=1,
+                      device=torch.cuda.current_device(), flags=args.kernel_flags) for _ in range(ns)]
+    main = torch.cuda.current_stream()
+
+    def streams_step():
+        n = 0
+        fork = torch.cuda.Event()
+        fork.record(main)
+        for sd in side:
+            sd.wait_event(fork)
+        for i, b0 in enumerate(range(0, T, cfg.batch)):
+            b1 = min(T, b0 + cfg.batch)
+            sctx[i % ns].encrypt_device(d_F[b0:b1], d_D[b0:b1], d_B[b0:b1], d_E[b0:b1], side[i % ns].cuda_stream)
+            n += sctx[i % ns].launch_count()[0]
+        for sd in side:
+            join = torch.cuda.Event()
+            join.record(sd)
+            main.wait_event(join)
+        return n
+
+    d_E.zero_()
+    torch.cuda.synchronize()
+    _t.sleep(idle_s)
+    for _ in range(2):
+        streams_step()
+    barrier()
+    sv = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    sv[0].record()
+    sl = 0
+    for _ in range(KB):
+        sl += streams_step()
+    sv[1].record()
+    barrier()
+    out["streams_ms_frame"] = sv[0].elapsed_time(sv[1]) / KB / T
+    out["streams_n"] = ns
+    out["streams_launches_per_step"] = sl // KB
+    out["streams_same"] = bool(synth.digest(d_E.cpu().numpy()) == out["digest_all"])
+    for v in sctx:
+        v.destroy()
 
     d_P = torch.empty_like(d_F)
     torch.cuda.synchronize()
@@ -373,6 +463,8 @@ def main():
     ap.add_argument("--no-extra-legs", action="store_true", help="skip the bounded C5 (4K) and C3 (single-frame latency) legs")
     ap.add_argument("--kernel-leg-only", action="store_true",
                     help="only the kernel-only legs, exactly --warmup untimed steps: the command profiles/ captures under ncu")
+    ap.add_argument("--direction", default="", choices=["", "encrypt", "decrypt"],
+                    help="with --kernel-leg-only: time only this direction (one call per step on the resident clip)")
     ap.add_argument("--clock-sample-ms", type=int, default=100, help="period of the nvidia-smi clock / throttle-reason samples")
     ap.add_argument("--persistent", action="store_true", help="kernel-only legs through the persistent kernel (VCRYPT_FLAG_PERSISTENT)")
     ap.add_argument("--derive", default="auto", choices=["auto", "host", "device"],
@@ -450,6 +542,14 @@ def main():
     kl = kernel_legs(args, cfg, vb, torch, T, d_F, d_D, d_B, K, W, barrier, sustained_ms=0.0 if args.kernel_leg_only else 1000.0)
     kern_ms_total = kl["total_ms"]
     pairs_per_step = max(1, kl["launches"] // (2 * K)) if not args.persistent else max(1, kl["launches"] // K)
+    if args.kernel_leg_only and args.direction:
+        if rank == 0:
+            print(json.dumps({"kernel_leg_only": True, "direction": kl["direction"], "config": cfg.name, "frames_per_step": T, "steps": K,
+                              "warmup_steps_run": kl["warm_steps"], "us_per_frame": 1e3 * kern_ms_total / K / T,
+                              "launches_per_step": kl["launches"] // K, "ok": kl["ok"]}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
     if args.kernel_leg_only:
         if rank == 0:
             print(json.dumps({"kernel_leg_only": True, "config": cfg.name, "frames_per_step": T, "steps": K, "warmup_steps_run": kl["warm_steps"],
@@ -557,6 +657,7 @@ def main():
     check["kernels_vs_e2e_first_frames"] = bool(kl["digest_first2"] == synth.digest(first_out[:2]))
     check["kernels_vs_e2e_all_frames"] = bool(kl["digest_all"] == first_all_digest)
     check["kernels_in_batches_same_bytes"] = kl["batches_same"]
+    check["kernels_in_batches_over_caller_streams_same_bytes"] = kl["streams_same"]
     check["decrypt_kernels_invert"] = kl["decrypt_ok"]
     check["e2e_decrypt_returns_clip"] = e2e_decrypt_ok
     if host_fps is not None:
@@ -574,7 +675,9 @@ def main():
     if not args.no_cpu_baseline:
         cpu_baseline = {"value": fps_or, "unit": UNIT, "cores": 1, "kind": "oracle",
                         "sample": f"first {n_or} frames of the clip, oracle/vcrypt_oracle.c single-threaded, "
-                                  f"{ncores} host cores present"}
+                                  f"{ncores} host cores present",
+                        # where the oracle's time goes (a second pass over the first frames, phases called one by one)
+                        "phases_ms_per_frame": time_oracle_phases(cfg, frames_np, min(4, n_or))}
 
     alg_bytes_frame = 3 * fb + 2 * nD  # read F_o + read B + write F_e + read D (~9wh)
     value = parallel.whole_job_rate(world, T, K, kern_ms_total * 1e-3)
@@ -583,6 +686,11 @@ def main():
     frames_per_pair = T / pairs_per_step
     traffic, col_share = ncu_traffic(cfg.name, frames_per_pair)
     batches_frac = alg_bytes_frame / (kl["batches_ms_frame"] * 1e-3) / 1e9 / peak
+    streams_frac = alg_bytes_frame / (kl["streams_ms_frame"] * 1e-3) / 1e9 / peak
+    sust = None
+    if "sustained_step_ms" in kl:
+        sust_gbs = alg_bytes_frame * T / (kl["sustained_step_ms"] * 1e-3) / 1e9
+        sust = {"value": world * T / (kl["sustained_step_ms"] * 1e-3), "gbs": sust_gbs, "frac": sust_gbs / peak}
     dec_frac = alg_bytes_frame / (kl["dec_ms_frame"] * 1e-3) / 1e9 / peak
     kernel_name = ("cipher_kernel (persistent: row team + strip team per SM)" if args.persistent else
                    "row_reg_kernel<false> + col_enc_kernel<64> = one launch pair of vcrypt_encrypt_device (col_enc_kernel is the larger "
@@ -599,8 +707,21 @@ def main():
         # headline against the nominal 8 TB/s the north star quotes: neither is hidden inside `roofline`
         "c4_batches_of_8_one_stream": {"value": 1e3 / kl["batches_ms_frame"], "unit": UNIT, "us_per_frame": 1e3 * kl["batches_ms_frame"],
                                        "frac": batches_frac, "frac_of_8TBs_nominal": batches_frac * peak / 8000.0},
+        # ... and literally as worded: the same batches round-robin over the config's 3 caller streams (one context per stream)
+        "c4_batches_of_8_three_streams": {"value": 1e3 / kl["streams_ms_frame"], "unit": UNIT, "us_per_frame": 1e3 * kl["streams_ms_frame"],
+                                          "n_streams": kl["streams_n"], "launches_per_step": kl["streams_launches_per_step"],
+                                          "frac": streams_frac, "frac_of_8TBs_nominal": streams_frac * peak / 8000.0,
+                                          "same_bytes": kl["streams_same"]},
         "frac_of_8TBs_nominal": achieved / 8000.0,
+        # `value` / roofline.frac are a burst from an idle GPU (like the measured copy peak); a video cipher runs continuously: the
+        # same step after a second of load, when the power cap has lowered the SM clock (rank 0's time x n_gpus under weak scaling)
+        "value_sustained": None if sust is None else sust["value"],
+        "frac_sustained": None if sust is None else sust["frac"],
         "targets": {"kernel_60pct_of_8TBs_nominal": {"met": bool(achieved / 8000.0 >= 0.6), "frac": achieved / 8000.0},
+                    "kernel_60pct_of_8TBs_nominal_sustained": None if sust is None else {"met": bool(sust["gbs"] / 8000.0 >= 0.6),
+                                                                                         "frac": sust["gbs"] / 8000.0},
+                    "kernel_60pct_of_measured_copy_rate_sustained": None if sust is None else {"met": bool(sust["frac"] >= 0.6),
+                                                                                              "frac": sust["frac"]},
                     "kernel_60pct_of_measured_copy_rate": {"met": bool(achieved / peak >= 0.6), "frac": achieved / peak},
                     "e2e_1000_frames_per_s": {"met": bool(e2e_value >= 1000.0), "value": e2e_value},
                     "bit_exact": {"met": True}},

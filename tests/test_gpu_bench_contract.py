@@ -36,6 +36,13 @@ def test_bench_prints_one_contract_line():
     assert set(t) >= {"kernel_60pct_of_8TBs_nominal", "kernel_60pct_of_measured_copy_rate", "e2e_1000_frames_per_s"}
     assert t["kernel_60pct_of_8TBs_nominal"]["met"] == (d["frac_of_8TBs_nominal"] >= 0.6)
     assert d["c4_batches_of_8_one_stream"]["frac"] > 0 and e["frac_of_pcie"] > 0 and e["pcie_copy_only"]["frames_per_s"] > e["value"]
+    # config 4 as worded (batches over 3 caller streams), the sustained figures at the top level, the oracle's phase split
+    s3 = d["c4_batches_of_8_three_streams"]
+    assert s3["frac"] > 0 and s3["n_streams"] == 3 and s3["same_bytes"] is True
+    assert d["value_sustained"] > 0 and 0 < d["frac_sustained"] < 1
+    assert t["kernel_60pct_of_8TBs_nominal_sustained"]["met"] == (t["kernel_60pct_of_8TBs_nominal_sustained"]["frac"] >= 0.6)
+    ph = cb["phases_ms_per_frame"]
+    assert ph["hash"] > 0 and ph["derivation"] > 0 and ph["confusion_xor"] > 0
 
 
 def test_bench_kernel_leg_only_line():
@@ -45,3 +52,9 @@ def test_bench_kernel_leg_only_line():
     assert r.returncode == 0, r.stderr[-2000:]
     d = json.loads([ln for ln in r.stdout.splitlines() if ln.strip()][-1])
     assert d["kernel_leg_only"] is True and d["ok"] is True and d["warmup_steps_run"] == 3 and d["us_per_frame"] > 0
+    for direction in ("encrypt", "decrypt"):
+        r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--config", "C2", "--steps", "1", "--warmup", "3", "--kernel-leg-only",
+                            "--direction", direction], capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        d = json.loads([ln for ln in r.stdout.splitlines() if ln.strip()][-1])
+        assert d["direction"] == direction and d["ok"] is True and d["us_per_frame"] > 0 and d["launches_per_step"] >= 2
