@@ -37,19 +37,19 @@ METRIC = "FHD frames/s encrypted"
 UNIT = "frames/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ALL kernels of one kernel-only step of this script, per launch
-# pair, from an ncu pass over `bench.py --kernel-leg-only` in the step's own configuration: one row per config, written by
-# hand from the capture named in profiles/r2_README.md
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
+# pair, from an ncu pass over `bench.py --kernel-leg-only` in the step's own configuration with the caches left as the run leaves
+# them: one row per config and direction, sums of the launch lists named in the file (profiles/r2_README.md, profiles/r3_README.md)
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r3_dram_traffic.csv")
 
 
-def ncu_traffic(cfg_name, frames_per_pair):
+def ncu_traffic(cfg_name, frames_per_pair, direction="encrypt"):
     """-> (DRAM bytes per launch pair, column pass's share of a pair's serialised time) for this config, or (None, None)."""
     try:
         import csv
 
         with open(TRAFFIC_FILE) as f:
             for row in csv.DictReader(f):
-                if row["config"] == cfg_name:
+                if row["config"] == cfg_name and row["direction"] == direction:
                     per_frame = (float(row["dram_read_bytes_per_step"]) + float(row["dram_write_bytes_per_step"])) / float(row["frames_per_step"])
                     return per_frame * frames_per_pair, float(row["column_pass_time_share"])
     except Exception:
@@ -386,6 +386,8 @@ def c5_leg(vb, torch, peak, frames=40, steps=3):
     res["frame_vs_oracle_ok"] = bool(np.array_equal(E[k].cpu().numpy(), O.confuse_xor(F[k].cpu().numpy(), D[k].cpu().numpy().view(np.uint16), B[k].cpu().numpy())))
     traffic, _ = ncu_traffic("C5", 1.0)
     res["traffic_per_frame"] = traffic
+    res["decrypt_traffic_per_frame"] = ncu_traffic("C5", 1.0, "decrypt")[0]
+    res["algorithmic_bytes_per_frame"] = alg
     v.destroy()
     return res
 
@@ -739,7 +741,7 @@ def main():
         "gpu_launches": kl["launches"],
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic,
-                     "traffic_source": "profiles/r2_dram_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum over all kernels of one step of "
+                     "traffic_source": "profiles/r3_dram_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum over all kernels of one step of "
                                        "`bench.py --kernel-leg-only` under ncu, per launch pair",
                      "kernel": kernel_name + f"; the step is ONE call on the resident clip = {pairs_per_step} launch pairs alternating over 2 "
                                "streams, so achieved = the step's algorithmic bytes / its duration (CUDA events on the calling stream, which the "
@@ -765,7 +767,8 @@ def main():
         "e2e_decrypt": {"value": world * T / min(dec_s), "unit": UNIT, "ms_per_frame": 1e3 * min(dec_s) / T,
                         "note": "vcrypt_decrypt_frames from the start of the chain, best of 3 after one warm-up call, pinned host in/out, rank 0's time"},
         "decrypt_kernels": {"value": 1e3 / kl["dec_ms_frame"], "unit": UNIT, "us_per_frame": 1e3 * kl["dec_ms_frame"],
-                            "frac": dec_frac, "steps": kl["dec_steps"]},
+                            "frac": dec_frac, "steps": kl["dec_steps"],
+                            "traffic_per_frame": ncu_traffic(cfg.name, 1.0, "decrypt")[0], "algorithmic_bytes_per_frame": alg_bytes_frame},
         "c5_4k_kernels": c5, "c3_single_frame_latency": c3,
         "cpu_baseline": cpu_baseline, "clocks": clocks, "check": check,
         "context": {"paper_ms_per_fhd_frame": 25.84, "paper_hw": "Xeon Gold 6226R + RTX 3090 (PAPER.md:5, :568); not a target"},

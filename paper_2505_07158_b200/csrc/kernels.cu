@@ -441,12 +441,17 @@ __global__ void __launch_bounds__(NT, MINB) row_reg_kernel(const uint8_t *src, u
 // columns x four byte lanes) and a sub-warp emits groups of 8 consecutive output rows with 64-bit
 // keystream loads and ciphertext stores.  Bank of a load = (strip row * X/4 + word column) mod 32 with strip
 // row = 4R + b: sub-warp s walks its columns in the order (word column a_l ^ (s & 1), byte lane a_b ^ (s >> 1)),
-// so the sub-warps of a warp sit in disjoint banks whatever rows they read -- that is the design intent for the GATHER
-// loads at X = 128, 64, 32.  It does not make the kernel conflict-free: the round-2 full capture
-// (profiles/r2_ncu_full_summary.csv) counts 185 K bank-conflict wavefronts out of 572 K shared-memory wavefronts per
-// launch of col_enc_kernel<64,256,2,2>, i.e. about half as many again as a conflict-free kernel would issue; which
-// instruction they belong to has not been attributed (no source-level capture yet).  The permutation is undone by the
-// selectors of the 4 x 4 byte transposes and by one select per output word.
+// so the sub-warps of a warp always sit in disjoint banks whatever rows they read: no conflicts for
+// X = 128, 64, 32.  The permutation is undone by the selectors of the 4 x 4 byte transposes and by one
+// select per output word.
+// Checked per instruction in round 3 (profiles/r3_source_summary.txt, from the source page of a full ncu capture):
+// every LDS / STS of col_enc_kernel and col_dec_kernel issues exactly its ideal number of wavefronts ("L1 Wavefronts
+// Shared Excessive" = 0 of 382 500 and of 870 300 per launch at FHD).  The hardware counter
+// l1tex__data_bank_conflicts_pipe_lsu_mem_shared that the kernel-level summary shows (186 K for col_enc_kernel, 507 K
+// for col_dec_kernel) is, to within 4 %, the number of shared-memory wavefronts that belong to NO instruction of the kernel
+// (575 K - 382.5 K = 193 K; 1 375 K - 870 K = 505 K): the TMA engine
+// writing the strip tiles (and, in the row kernels, the bulk stores reading the output buffer).  ncu counts that
+// async-proxy traffic in the same pipe counter; it is not a conflict between the threads' accesses.
 // In place is safe: the whole strip is in shared memory before the first store.
 // ---------------------------------------------------------------------------------------------
 // keystream prefetch depths (rounds of loads in flight per thread): decrypt column pass with three CTAs per SM / one CTA per
